@@ -1,0 +1,158 @@
+/* hough.h -- C ABI of libhough: batched Hough-transform track finding on one B200 (sm_100a).
+ *
+ * The hot path of arxiv 2511.02742 ("GPU-based track-finding for the J-PARC muon g-2/EDM experiment"):
+ *
+ *   vote      every hit (u, v) adds one entry per theta bin to a 2-D histogram over (theta, rho),
+ *             rho = u cos(theta) + v sin(theta)                       PAPER.md L90-92 (Sec. 4, Eq. 4.1)
+ *             theta in [0, 180 deg), rho binned over a fixed range      PAPER.md L106 (Sec. 5)
+ *   peaks     "the bin with the highest number of entries", here every strict local maximum with
+ *             at least `vote_threshold` entries; clusters are the 8-connected components of the
+ *             thresholded histogram                                   PAPER.md L94, L106; keyword L29
+ *   assign    "selecting the hits that align with the straight line formed by the identified
+ *             (theta, rho)"
+ *
+ * The paper fills one histogram per 10 ns time window in the shared memory of one CUDA block
+ * (PAPER.md L114-116); an "event" here is one such window's 2-D point set.  Bin indices are computed
+ * in fixed-point integer arithmetic from cos/sin tables defined by formula, so
+ * every output except the two fp32 line parameters is an exact integer result.
+ *
+ * Conventions
+ *   - d_* pointers are caller-owned DEVICE memory, h_* pointers are caller-owned HOST memory.  The library
+ *     never keeps them past the call's stream work.  `stream` is a cudaStream_t passed as void* (NULL = the
+ *     legacy default stream).
+ *   - hough_vote / hough_find_clusters / hough_assign_hits only enqueue work on `stream`: no host
+ *     synchronisation, no allocation.  Calls on one plan must be issued on one stream at a time (the plan
+ *     owns scratch memory that the kernels reuse).
+ *   - Return value: HOUGH_OK (0) or a negative hough_status code.  Nothing throws or aborts across the ABI.
+ *   - Data-dependent conditions are not errors: an event with more than K local maxima reports the
+ *     untruncated count in n_found and writes only the first K records; invalid hits (non-finite, or
+ *     |u| or |v| > coord_max) cast no votes and get label -1; an event longer than max_hits_per_event or
+ *     with decreasing offsets is skipped (no candidates, labels -1) and sets a bit in the plan's device
+ *     status word (hough_plan_status).
+ */
+#ifndef HOUGH_H_
+#define HOUGH_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    HOUGH_OK = 0,
+    HOUGH_EINVAL = -1,  /* null pointer, negative size, misaligned buffer, bad descriptor field            */
+    HOUGH_ERANGE = -2,  /* grid / fixed-point parameters fail the int32 proof, or a size exceeds the plan  */
+    HOUGH_ECUDA = -3,   /* a CUDA runtime call failed; see hough_last_cuda_error()                         */
+    HOUGH_ENOMEM = -4   /* host or device allocation failed                                                */
+} hough_status;
+
+enum { HOUGH_I32 = 0, HOUGH_U16 = 1 };            /* count_dtype: element type of accumulators dumped by hough_vote */
+enum { HOUGH_STATUS_EVENT_TOO_LONG = 1, HOUGH_STATUS_BAD_OFFSETS = 2 };   /* bits of the device status word */
+
+typedef struct hough_plan hough_plan_t;           /* opaque; created and destroyed by the library */
+
+/* The (theta, rho) grid, thresholds and capacities of one plan.
+ * theta always spans [0, pi): bin t stands for theta_t = pi t / n_theta (left edge; "0 to 180 deg").
+ * rho spans the half-open range [rho_min, rho_max) in n_rho equal bins (histogram semantics). */
+typedef struct {
+    int32_t n_theta, n_rho;       /* >= 1; n_theta * n_rho <= 2^22                                          */
+    double rho_min, rho_max;      /* same length unit as the hits                                           */
+    double coord_max;             /* a hit is valid iff finite and |u|, |v| <= coord_max                    */
+    int32_t hit_frac_bits;        /* H: hits are rounded to multiples of 2^-H (ties to even); < 0 -> 6      */
+    int32_t acc_frac_bits;        /* F: fraction bits of the fixed-point rho bin coordinate; < 0 -> largest
+                                     F <= 24 that keeps every intermediate inside int32                    */
+    int32_t vote_threshold;       /* T >= 1: a bin is "on" iff its count >= T                               */
+    double assign_window;         /* w >= 0, in rho units: a hit may join a candidate iff its distance to
+                                     the candidate's bin-centre line is <= w                               */
+    int32_t max_candidates;       /* K in [1, 4096]: records kept per event                                 */
+    int32_t count_dtype;          /* HOUGH_I32 or HOUGH_U16                                                 */
+    int32_t max_events;           /* capacity: events per call                                              */
+    int64_t max_hits;             /* capacity: hits per call                                                */
+    int32_t max_hits_per_event;   /* capacity: hits in one event (HOUGH_U16 needs <= 65535)                 */
+    int32_t flags;                /* reserved, 0                                                            */
+    int32_t device;               /* CUDA device ordinal                                                    */
+} hough_plan_desc_t;
+
+/* One track candidate: a local maximum of the event's accumulator.  32 bytes, little endian. */
+typedef struct {
+    int32_t theta_bin, rho_bin;   /* the peak bin (t, r)                                                    */
+    int32_t votes;                /* its count                                                              */
+    int32_t cluster_root;         /* slot, in this event's list, of the best-ranked peak of its cluster     */
+    int32_t cluster_nbins;        /* bins in the 8-connected cluster (count >= T) that contains the peak    */
+    float theta, rho;             /* line parameters of the bin: theta_t, and the rho bin centre            */
+    int32_t reserved;             /* 0                                                                      */
+} hough_candidate_t;
+
+/* Constants a plan derived from its descriptor; for tests and diagnostics. */
+typedef struct {
+    int32_t hit_frac_bits, acc_frac_bits;  /* H, F                                                          */
+    int32_t rho_offset_q;                  /* O_q = llround(-rho_min 2^F / d_rho)                           */
+    int32_t assign_window_q;               /* W_q = llround(w 2^F / d_rho)                                  */
+    int32_t strip_rows, n_strips;          /* theta rows of one shared-memory tile; tiles per event         */
+    int32_t counter_bytes;                 /* width of the shared-memory counters (2 or 4)                  */
+    int32_t threads_per_cta, ctas_per_sm, n_ctas, smem_bytes_per_cta;
+    int32_t n_sm;
+} hough_plan_info_t;
+
+/* Validate the descriptor, derive F, build the int32 cos/sin tables C_q[t] = llround(cos(theta_t) M),
+ * S_q[t] = llround(sin(theta_t) M), M = 2^(F-H) / d_rho, upload them, allocate scratch.  *out is set only on success. */
+int hough_plan_create(const hough_plan_desc_t* desc, hough_plan_t** out);
+
+/* Frees everything the plan owns.  Synchronises the device.  NULL is allowed. */
+int hough_plan_destroy(hough_plan_t* plan);
+
+/* Histogram filling only (Eq. 4.1): the materialising / diagnostic path.
+ *   d_u, d_v      [N] fp32 hit coordinates, structure of arrays, 16-byte aligned
+ *   d_offsets     [n_events + 1] int64, event e owns hits [offsets[e], offsets[e+1]); offsets[0] >= 0
+ *   d_acc         nullable; [n_events][n_theta][n_rho] of count_dtype, theta-major, fully overwritten
+ *   d_digest      nullable; [n_events] uint64: sum over bins of count * splitmix64(t * n_rho + r) mod 2^64 */
+int hough_vote(hough_plan_t* plan, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events,
+               void* d_acc, uint64_t* d_digest, void* stream);
+
+/* Vote + peak/cluster finding, fused: the accumulator lives only in shared memory.
+ *   d_cands       [n_events][K] records; event e gets min(n_found[e], K) records in rank order
+ *                 (votes descending, then t * n_rho + r ascending); the rest of its row is left untouched
+ *   d_n_found     [n_events] int32: number of local maxima >= T of the event, not truncated to K */
+int hough_find_clusters(hough_plan_t* plan, const float* d_u, const float* d_v, const int64_t* d_offsets,
+                        int32_t n_events, hough_candidate_t* d_cands, int32_t* d_n_found, void* stream);
+
+/* Hit-to-candidate assignment: label[h] = slot of the kept candidate whose bin-centre line is
+ * nearest to hit h (fixed-point residual at the candidate's theta), among those within the window; ties go to
+ * the lower slot; -1 if none or if the hit is invalid.
+ *   d_cands, d_n_found   as written by hough_find_clusters for the same events
+ *   d_labels             [N] int32, every element of the events' ranges is written */
+int hough_assign_hits(hough_plan_t* plan, const float* d_u, const float* d_v, const int64_t* d_offsets,
+                      int32_t n_events, const hough_candidate_t* d_cands, const int32_t* d_n_found,
+                      int32_t* d_labels, void* stream);
+
+/* ---- helpers beyond the five ---- */
+
+/* hough_find_clusters + hough_assign_hits on HOST buffers: copies u, v, offsets to the device, runs both
+ * kernels, copies cands, n_found and labels back, and synchronises.  h_offsets[0] must be 0 and
+ * h_offsets[n_events] the number of hits.  Any output pointer may be NULL (then it is not copied back). */
+int hough_run_host(hough_plan_t* plan, const float* h_u, const float* h_v, const int64_t* h_offsets,
+                   int32_t n_events, hough_candidate_t* h_cands, int32_t* h_n_found, int32_t* h_labels);
+
+/* Derived constants; h_cos_q / h_sin_q are nullable host arrays of n_theta int32 that receive the tables. */
+int hough_plan_query(const hough_plan_t* plan, hough_plan_info_t* info, int32_t* h_cos_q, int32_t* h_sin_q);
+
+/* Reads and clears the device status word (HOUGH_STATUS_* bits).  Synchronises `stream`. */
+int hough_plan_status(hough_plan_t* plan, int32_t* out, void* stream);
+
+/* Number of kernels the library has launched through this plan since creation. */
+int64_t hough_plan_launch_count(const hough_plan_t* plan);
+
+/* Measures the conflict-free shared-memory atomic-add rate of the device (the roofline denominator of the
+ * vote kernel): every SM runs `red.shared.add.u32` with lane = bank for about `millis` ms.
+ * *ops_per_s receives the rate over the whole chip, *sm_clock_mhz the SM clock seen meanwhile. */
+int hough_measure_smem_atomic_peak(int32_t device, double millis, double* ops_per_s, double* sm_clock_mhz);
+
+const char* hough_strerror(int status);
+const char* hough_last_cuda_error(void);          /* text of the last failed CUDA call on this thread, or "" */
+int hough_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HOUGH_H_ */

@@ -1,0 +1,503 @@
+// hough_lib.cu -- host side of libhough: the C ABI of include/hough.h over the kernels of hough_kernels.cuh.
+//
+// No torch, no Python: plain CUDA runtime.  Built for sm_100a only (see paper_2511_02742_b200/build.py).
+#include "../../include/hough.h"
+#include "hough_kernels.cuh"
+
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+using hough::Candidate;
+using hough::DevParams;
+
+static_assert(sizeof(hough_candidate_t) == 32, "record layout");
+static_assert(sizeof(Candidate) == sizeof(hough_candidate_t), "device record mirrors the ABI record");
+
+static thread_local char g_cuda_err[256] = "";
+
+static int cuda_fail(cudaError_t e, const char* what)
+{
+    snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s", what, cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    return HOUGH_ECUDA;
+}
+#define HCK(call)                                                   \
+    do {                                                            \
+        cudaError_t e_ = (call);                                    \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);         \
+    } while (0)
+
+struct hough_plan {
+    hough_plan_desc_t desc;
+    DevParams P;
+    hough_plan_info_t info;
+    std::vector<int32_t> h_cos, h_sin;
+    int cw, G;  // counter bytes, column groups per tile
+    int n_ctas, threads, smem_bytes;
+    int assign_ctas;
+    int64_t launches;
+    // owned device memory
+    int* d_cos;
+    int* d_sin;
+    void* d_scratch;
+    int* d_status;
+    unsigned int* d_counter;
+    // lazily created resources of hough_run_host
+    cudaStream_t h_stream;
+    float* hd_u;
+    float* hd_v;
+    long long* hd_off;
+    Candidate* hd_cands;
+    int* hd_nfound;
+    int* hd_labels;
+};
+
+static int env_int(const char* name, int dflt)
+{
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Shared-memory footprint of everything but the tile.
+struct SmemLayout {
+    int off_hits, off_halo, off_peaks, off_kept, off_kroot, off_hist, total;
+};
+static SmemLayout layout_smem(int tile_bytes, int HB, int n_rho, int PCAP, int K)
+{
+    SmemLayout L;
+    size_t o = align_up((size_t)tile_bytes, 1024);
+    L.off_hits = (int)o;   o = align_up(o + (size_t)HB * 8, 16);
+    L.off_halo = (int)o;   o = align_up(o + (size_t)2 * n_rho * 4, 16);
+    L.off_peaks = (int)o;  o = align_up(o + (size_t)PCAP * 8, 16);
+    L.off_kept = (int)o;   o = align_up(o + (size_t)2 * K * 8, 16);
+    L.off_kroot = (int)o;  o = align_up(o + (size_t)K * 4, 16);
+    L.off_hist = (int)o;   o = align_up(o + 256 * 4, 16);
+    L.total = (int)o;
+    return L;
+}
+
+template <int CW, int G, bool DUMP>
+static cudaError_t launch_event_kernel(const hough_plan* p, const float* u, const float* v, const long long* off, int n_events,
+                                       Candidate* cands, int* n_found, void* acc, int acc_u16, unsigned long long* digest,
+                                       cudaStream_t st)
+{
+    auto k = hough::hough_event_kernel<CW, G, DUMP>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes);
+    if (e != cudaSuccess) return e;
+    k<<<p->n_ctas, p->threads, p->smem_bytes, st>>>(p->P, u, v, off, n_events, cands, n_found, acc, acc_u16, digest);
+    return cudaGetLastError();
+}
+
+template <bool DUMP>
+static cudaError_t dispatch_event_kernel(const hough_plan* p, const float* u, const float* v, const long long* off, int n_events,
+                                         Candidate* cands, int* n_found, void* acc, int acc_u16, unsigned long long* digest,
+                                         cudaStream_t st)
+{
+#define HOUGH_CASE(CW_, G_)                                                                                                 \
+    if (p->cw == CW_ && p->G == G_)                                                                                         \
+        return launch_event_kernel<CW_, G_, DUMP>(p, u, v, off, n_events, cands, n_found, acc, acc_u16, digest, st);
+    HOUGH_CASE(2, 1) HOUGH_CASE(2, 2) HOUGH_CASE(2, 3) HOUGH_CASE(2, 4) HOUGH_CASE(2, 6) HOUGH_CASE(2, 8)
+    HOUGH_CASE(4, 1) HOUGH_CASE(4, 2) HOUGH_CASE(4, 3) HOUGH_CASE(4, 4) HOUGH_CASE(4, 6) HOUGH_CASE(4, 8)
+#undef HOUGH_CASE
+    return cudaErrorInvalidValue;
+}
+
+static const int kGroupChoices[] = {8, 6, 4, 3, 2, 1};
+
+extern "C" {
+
+int hough_version(void) { return 100; }
+
+const char* hough_strerror(int s)
+{
+    switch (s) {
+        case HOUGH_OK: return "ok";
+        case HOUGH_EINVAL: return "invalid argument";
+        case HOUGH_ERANGE: return "parameter outside the supported range (int32 proof or plan capacity)";
+        case HOUGH_ECUDA: return "CUDA error";
+        case HOUGH_ENOMEM: return "out of memory";
+        default: return "unknown status";
+    }
+}
+
+const char* hough_last_cuda_error(void) { return g_cuda_err; }
+
+int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
+{
+    if (!d || !out) return HOUGH_EINVAL;
+    if (d->n_theta < 1 || d->n_rho < 1 || !(d->rho_max > d->rho_min) || !isfinite(d->rho_min) || !isfinite(d->rho_max)) return HOUGH_EINVAL;
+    if (!(d->coord_max > 0) || !isfinite(d->coord_max)) return HOUGH_EINVAL;
+    if (d->vote_threshold < 1 || !(d->assign_window >= 0) || !isfinite(d->assign_window)) return HOUGH_EINVAL;
+    if (d->max_candidates < 1 || d->max_candidates > 4096) return HOUGH_EINVAL;
+    if (d->count_dtype != HOUGH_I32 && d->count_dtype != HOUGH_U16) return HOUGH_EINVAL;
+    if (d->max_events < 1 || d->max_hits < 0 || d->max_hits_per_event < 0 || d->device < 0) return HOUGH_EINVAL;
+    if (d->count_dtype == HOUGH_U16 && d->max_hits_per_event > 65535) return HOUGH_ERANGE;  // a bin gets <= 1 vote per hit
+    if ((int64_t)d->n_theta * d->n_rho > (1ll << hough::kLBits)) return HOUGH_ERANGE;
+    const int H = d->hit_frac_bits < 0 ? 6 : d->hit_frac_bits;
+    if (H > 20) return HOUGH_ERANGE;
+
+    // ---- fixed-point constants (host double precision, llround = half away from zero)
+    const double d_rho = (d->rho_max - d->rho_min) / d->n_rho;
+    int F = d->acc_frac_bits;
+    if (F < 0) {
+        const double amin = fabs(d->rho_min), amax = fabs(d->rho_max);
+        const double span = sqrt(2.0) * d->coord_max / d_rho + (amin > amax ? amin : amax) / d_rho + 2.0;
+        F = 24;
+        while (F > 0 && span * ldexp(1.0, F) > 2147483647.0) --F;
+    }
+    if (F > 30 || F < 1) return HOUGH_ERANGE;
+    const double M = ldexp(1.0, F - H) / d_rho;
+    const double oq_d = -d->rho_min * ldexp(1.0, F) / d_rho;
+    const double wq_d = d->assign_window * ldexp(1.0, F) / d_rho;
+    if (fabs(oq_d) > 2147483646.0 || wq_d > 2147483646.0 || M > 2147483646.0) return HOUGH_ERANGE;
+    const long long Oq = llround(oq_d), Wq = llround(wq_d);
+
+    hough_plan* p = new (std::nothrow) hough_plan();
+    if (!p) return HOUGH_ENOMEM;
+    p->desc = *d;
+    p->desc.hit_frac_bits = H;
+    p->desc.acc_frac_bits = F;
+    p->h_cos.resize(d->n_theta);
+    p->h_sin.resize(d->n_theta);
+    long long max_cs = 0;
+    for (int t = 0; t < d->n_theta; ++t) {
+        const double th = 3.14159265358979323846 * t / d->n_theta;
+        const long long c = llround(cos(th) * M), s = llround(sin(th) * M);
+        p->h_cos[t] = (int32_t)c;
+        p->h_sin[t] = (int32_t)s;
+        const long long cs = llabs(c) + llabs(s);
+        if (cs > max_cs) max_cs = cs;
+    }
+    // int32 proof: |u_q C| + |v_q S| + |O_q| <= 2^31 - 1 for every valid hit, and bin centres r 2^F + 2^(F-1) fit too
+    const long long qmax = (long long)floor(d->coord_max * ldexp(1.0, H)) + 1;
+    if ((double)qmax * (double)max_cs + fabs((double)Oq) > 2147483647.0 || ((double)d->n_rho + 1.0) * ldexp(1.0, F) > 2147483647.0) {
+        delete p;
+        return HOUGH_ERANGE;
+    }
+
+    // ---- launch configuration
+    int dev_count = 0;
+    cudaError_t ce = cudaGetDeviceCount(&dev_count);
+    if (ce != cudaSuccess || d->device >= dev_count) { delete p; return ce != cudaSuccess ? cuda_fail(ce, "cudaGetDeviceCount") : HOUGH_EINVAL; }
+    cudaDeviceProp prop;
+    if ((ce = cudaSetDevice(d->device)) != cudaSuccess || (ce = cudaGetDeviceProperties(&prop, d->device)) != cudaSuccess) {
+        delete p;
+        return cuda_fail(ce, "cudaGetDeviceProperties");
+    }
+    const int n_sm = prop.multiProcessorCount;
+    const int smem_optin = (int)prop.sharedMemPerBlockOptin;            // 227 KiB on B200
+    const int smem_sm = (int)prop.sharedMemPerMultiprocessor;           // 228 KiB
+    const int reserved = (int)prop.reservedSharedMemPerBlock;           // 1 KiB
+
+    int cw = (d->max_hits_per_event <= 65535 && d->vote_threshold <= 65535) ? 2 : 4;
+    const int cw_env = env_int("HOUGH_COUNTER_BYTES", 0);
+    if (cw_env == 4) cw = 4;
+    const int rpg = 32 * (4 / cw);  // theta rows per column group
+    const int groups_all = (d->n_theta + rpg - 1) / rpg;
+    const int K = d->max_candidates;
+    const int HB = (int)align_up((size_t)(d->max_hits_per_event < 32 ? 32 : (d->max_hits_per_event > 4096 ? 4096 : d->max_hits_per_event)), 32);
+
+    int ctas_per_sm = env_int("HOUGH_CTAS_PER_SM", 0);
+    int threads = env_int("HOUGH_THREADS", 0);
+    int G = env_int("HOUGH_GROUPS", 0);
+    auto fits = [&](int g, int cps, int pcap) {
+        // 256 bytes of headroom for the kernel's static shared variables
+        const int budget = (cps == 1 ? smem_optin : (smem_sm / cps - reserved)) - 256;
+        return layout_smem(d->n_rho * 128 * g, HB, d->n_rho, pcap, K).total <= (budget < smem_optin ? budget : smem_optin);
+    };
+    int g_cover = 8;  // smallest choice that covers every theta row (no point in allocating rows beyond n_theta)
+    for (int g : kGroupChoices) if (g >= groups_all) g_cover = g;
+    auto pick_G = [&](int cps) {
+        for (int g : kGroupChoices)
+            if (g <= g_cover && fits(g, cps, 512)) return g;
+        return 0;
+    };
+    if (ctas_per_sm <= 0) {
+        // default: two CTAs per SM when a tile of at least two column groups (or the whole grid) still fits, so that one
+        // CTA's scan / cluster phases overlap the other's voting; otherwise one large CTA
+        const int g2 = pick_G(2);
+        ctas_per_sm = (g2 >= 2 || (g2 >= 1 && g2 >= groups_all)) ? 2 : 1;
+    }
+    if (G <= 0) G = pick_G(ctas_per_sm);
+    if (G <= 0 && ctas_per_sm > 1) { ctas_per_sm = 1; G = pick_G(1); }
+    if (G <= 0 || !fits(G, ctas_per_sm, 256)) { delete p; return HOUGH_ERANGE; }
+    if (threads <= 0) threads = ctas_per_sm == 1 ? 1024 : 512;
+    threads = threads / 32 * 32;
+    if (threads < 32 || threads > hough::kMaxThreads) { delete p; return HOUGH_EINVAL; }
+    int PCAP = 4096;
+    while (PCAP > 256 && !fits(G, ctas_per_sm, PCAP)) PCAP -= 256;
+    const int S = G * rpg;
+    const int n_strips = (d->n_theta + S - 1) / S;
+    const int tile_bytes = d->n_rho * 128 * G;
+    const SmemLayout lay = layout_smem(tile_bytes, HB, d->n_rho, PCAP, K);
+
+    p->cw = cw;
+    p->G = G;
+    p->threads = threads;
+    p->smem_bytes = lay.total;
+    p->n_ctas = n_sm * ctas_per_sm;
+    p->assign_ctas = n_sm * 8;
+    p->launches = 0;
+
+    // ---- device memory
+    const size_t n_bins = (size_t)d->n_theta * d->n_rho;
+    const size_t tab = (size_t)n_strips * S;
+    const size_t per_cta = n_bins * 4 + n_bins * 4 + n_bins * 8 + (n_bins / 4 + 1) * 8 + 16;
+    const size_t scratch_bytes = align_up(per_cta, 256) * p->n_ctas + 256;
+    std::vector<int32_t> padc(tab, 0), pads(tab, 0);
+    memcpy(padc.data(), p->h_cos.data(), sizeof(int32_t) * d->n_theta);
+    memcpy(pads.data(), p->h_sin.data(), sizeof(int32_t) * d->n_theta);
+    bool ok = true;
+    ok = ok && (ce = cudaMalloc((void**)&p->d_cos, tab * 4)) == cudaSuccess;
+    ok = ok && (ce = cudaMalloc((void**)&p->d_sin, tab * 4)) == cudaSuccess;
+    ok = ok && (ce = cudaMalloc(&p->d_scratch, scratch_bytes)) == cudaSuccess;
+    ok = ok && (ce = cudaMalloc((void**)&p->d_status, 256)) == cudaSuccess;
+    ok = ok && (ce = cudaMemcpy(p->d_cos, padc.data(), tab * 4, cudaMemcpyHostToDevice)) == cudaSuccess;
+    ok = ok && (ce = cudaMemcpy(p->d_sin, pads.data(), tab * 4, cudaMemcpyHostToDevice)) == cudaSuccess;
+    ok = ok && (ce = cudaMemset(p->d_scratch, 0, scratch_bytes)) == cudaSuccess;
+    ok = ok && (ce = cudaMemset(p->d_status, 0, 256)) == cudaSuccess;
+    if (!ok) {
+        const int rc = (ce == cudaErrorMemoryAllocation) ? HOUGH_ENOMEM : cuda_fail(ce, "plan allocation");
+        (void)cudaGetLastError();
+        hough_plan_destroy(p);
+        return rc;
+    }
+    p->d_counter = reinterpret_cast<unsigned int*>(p->d_status) + 16;
+
+    DevParams& P = p->P;
+    memset(&P, 0, sizeof P);
+    P.n_theta = d->n_theta; P.n_rho = d->n_rho; P.n_bins = (int)n_bins;
+    P.F = F; P.H = H; P.Oq = (int)Oq; P.Wq = (int)Wq; P.T = d->vote_threshold; P.K = K;
+    P.coord_max = (float)d->coord_max;
+    // fp32 compare |u| <= coord_max must equal the double compare of the definition: round coord_max DOWN to fp32
+    if ((double)P.coord_max > d->coord_max) P.coord_max = nextafterf(P.coord_max, 0.0f);
+    P.hit_scale = ldexpf(1.0f, H);
+    {
+        // safe radius: R (M + 1) <= min(O_q, n_rho 2^F - 1 - O_q)  =>  0 <= a < n_rho 2^F for every theta (Cauchy-Schwarz)
+        const double lo = (double)Oq, hi = (double)d->n_rho * ldexp(1.0, F) - 1.0 - (double)Oq;
+        const double m = lo < hi ? lo : hi;
+        if (m > 0) {
+            const double R = m / (M + 1.0);
+            const double r2 = floor(R * R * (1.0 - 1e-9)) - 1.0;
+            P.safe_enabled = r2 >= 0;
+            P.r2safe = r2 >= 0 ? (unsigned long long)r2 : 0;
+        }
+        if (env_int("HOUGH_NO_SAFE_PATH", 0)) P.safe_enabled = 0;
+    }
+    P.S = S; P.n_strips = n_strips; P.row_bytes = 128 * G; P.tile_bytes = tile_bytes;
+    P.HB = HB; P.PCAP = PCAP;
+    P.max_hits_per_event = d->max_hits_per_event;
+    P.rho_min = d->rho_min; P.d_rho = d_rho;
+    P.Cq = p->d_cos; P.Sq = p->d_sin;
+    P.off_hits = lay.off_hits; P.off_halo = lay.off_halo; P.off_peaks = lay.off_peaks;
+    P.off_kept = lay.off_kept; P.off_kroot = lay.off_kroot; P.off_hist = lay.off_hist;
+    {
+        unsigned char* b = static_cast<unsigned char*>(p->d_scratch);
+        const size_t nc = (size_t)p->n_ctas;
+        P.parent = reinterpret_cast<uint32_t*>(b);              b += align_up(n_bins * 4 * nc, 256);
+        P.csize = reinterpret_cast<uint32_t*>(b);               b += align_up(n_bins * 4 * nc, 256);
+        P.onlist = reinterpret_cast<uint2*>(b);                 b += align_up(n_bins * 8 * nc, 256);
+        P.peaks_ovf = reinterpret_cast<uint2*>(b);              b += align_up((n_bins / 4 + 1) * 8 * nc, 256);
+        P.epoch = reinterpret_cast<uint32_t*>(b);
+        if ((size_t)(b - static_cast<unsigned char*>(p->d_scratch)) + nc * 4 > scratch_bytes) { hough_plan_destroy(p); return HOUGH_ENOMEM; }
+    }
+    P.status = p->d_status;
+    P.work_counter = p->d_counter;
+
+    hough_plan_info_t& I = p->info;
+    I.hit_frac_bits = H; I.acc_frac_bits = F; I.rho_offset_q = (int32_t)Oq; I.assign_window_q = (int32_t)Wq;
+    I.strip_rows = S; I.n_strips = n_strips; I.counter_bytes = cw;
+    I.threads_per_cta = threads; I.ctas_per_sm = ctas_per_sm; I.n_ctas = p->n_ctas; I.smem_bytes_per_cta = lay.total;
+    I.n_sm = n_sm;
+    *out = p;
+    return HOUGH_OK;
+}
+
+int hough_plan_destroy(hough_plan_t* p)
+{
+    if (!p) return HOUGH_OK;
+    (void)cudaSetDevice(p->desc.device);
+    (void)cudaDeviceSynchronize();
+    cudaFree(p->d_cos); cudaFree(p->d_sin); cudaFree(p->d_scratch); cudaFree(p->d_status);
+    cudaFree(p->hd_u); cudaFree(p->hd_v); cudaFree(p->hd_off); cudaFree(p->hd_cands); cudaFree(p->hd_nfound); cudaFree(p->hd_labels);
+    if (p->h_stream) cudaStreamDestroy(p->h_stream);
+    (void)cudaGetLastError();
+    delete p;
+    return HOUGH_OK;
+}
+
+int hough_plan_query(const hough_plan_t* p, hough_plan_info_t* info, int32_t* h_cos_q, int32_t* h_sin_q)
+{
+    if (!p) return HOUGH_EINVAL;
+    if (info) *info = p->info;
+    if (h_cos_q) memcpy(h_cos_q, p->h_cos.data(), sizeof(int32_t) * p->h_cos.size());
+    if (h_sin_q) memcpy(h_sin_q, p->h_sin.data(), sizeof(int32_t) * p->h_sin.size());
+    return HOUGH_OK;
+}
+
+int64_t hough_plan_launch_count(const hough_plan_t* p) { return p ? p->launches : 0; }
+
+int hough_plan_status(hough_plan_t* p, int32_t* out, void* stream)
+{
+    if (!p || !out) return HOUGH_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(p->desc.device));
+    HCK(cudaMemcpyAsync(out, p->d_status, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    HCK(cudaMemsetAsync(p->d_status, 0, sizeof(int32_t), st));
+    HCK(cudaStreamSynchronize(st));
+    return HOUGH_OK;
+}
+
+static int check_common(const hough_plan_t* p, const float* u, const float* v, const int64_t* off, int32_t n_events)
+{
+    if (!p || !off || n_events < 0) return HOUGH_EINVAL;
+    if (n_events > p->desc.max_events) return HOUGH_ERANGE;
+    // u, v may be null for a batch without hits (an empty tensor has no storage); they are never read then
+    if (((uintptr_t)u & 15) || ((uintptr_t)v & 15) || ((uintptr_t)off & 7)) return HOUGH_EINVAL;
+    return HOUGH_OK;
+}
+
+int hough_vote(hough_plan_t* p, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events, void* d_acc,
+               uint64_t* d_digest, void* stream)
+{
+    int rc = check_common(p, d_u, d_v, d_offsets, n_events);
+    if (rc) return rc;
+    if (n_events == 0 || (!d_acc && !d_digest)) return HOUGH_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(p->desc.device));
+    HCK(cudaMemsetAsync(p->d_counter, 0, sizeof(unsigned int), st));
+    HCK(dispatch_event_kernel<true>(p, d_u, d_v, reinterpret_cast<const long long*>(d_offsets), n_events, nullptr, nullptr, d_acc,
+                                    p->desc.count_dtype == HOUGH_U16, reinterpret_cast<unsigned long long*>(d_digest), st));
+    p->launches += 1;
+    return HOUGH_OK;
+}
+
+int hough_find_clusters(hough_plan_t* p, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events,
+                        hough_candidate_t* d_cands, int32_t* d_n_found, void* stream)
+{
+    int rc = check_common(p, d_u, d_v, d_offsets, n_events);
+    if (rc) return rc;
+    if (!d_cands || !d_n_found) return HOUGH_EINVAL;
+    if (((uintptr_t)d_cands & 15) || ((uintptr_t)d_n_found & 3)) return HOUGH_EINVAL;
+    if (n_events == 0) return HOUGH_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(p->desc.device));
+    HCK(cudaMemsetAsync(p->d_counter, 0, sizeof(unsigned int), st));
+    HCK(dispatch_event_kernel<false>(p, d_u, d_v, reinterpret_cast<const long long*>(d_offsets), n_events,
+                                     reinterpret_cast<Candidate*>(d_cands), d_n_found, nullptr, 0, nullptr, st));
+    p->launches += 1;
+    return HOUGH_OK;
+}
+
+int hough_assign_hits(hough_plan_t* p, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events,
+                      const hough_candidate_t* d_cands, const int32_t* d_n_found, int32_t* d_labels, void* stream)
+{
+    int rc = check_common(p, d_u, d_v, d_offsets, n_events);
+    if (rc) return rc;
+    if (!d_cands || !d_n_found) return HOUGH_EINVAL;
+    if (n_events == 0) return HOUGH_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(p->desc.device));
+    const int grid = n_events < p->assign_ctas ? n_events : p->assign_ctas;
+    if ((size_t)p->P.K * 16 > 48 * 1024)
+        HCK(cudaFuncSetAttribute(hough::hough_assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, p->P.K * 16));
+    hough::hough_assign_kernel<<<grid, 256, (size_t)p->P.K * 16, st>>>(p->P, d_u, d_v, reinterpret_cast<const long long*>(d_offsets),
+                                                                      n_events, reinterpret_cast<const Candidate*>(d_cands),
+                                                                      d_n_found, d_labels);
+    HCK(cudaGetLastError());
+    p->launches += 1;
+    return HOUGH_OK;
+}
+
+int hough_run_host(hough_plan_t* p, const float* h_u, const float* h_v, const int64_t* h_offsets, int32_t n_events,
+                   hough_candidate_t* h_cands, int32_t* h_n_found, int32_t* h_labels)
+{
+    if (!p || !h_offsets || n_events < 0) return HOUGH_EINVAL;
+    if (n_events > p->desc.max_events) return HOUGH_ERANGE;
+    if (n_events == 0) return HOUGH_OK;
+    if (h_offsets[0] != 0) return HOUGH_EINVAL;
+    const int64_t n_hits = h_offsets[n_events];
+    if (n_hits < 0 || (n_hits > 0 && (!h_u || !h_v))) return HOUGH_EINVAL;
+    if (n_hits > p->desc.max_hits) return HOUGH_ERANGE;
+    HCK(cudaSetDevice(p->desc.device));
+    if (!p->h_stream) {
+        const size_t mh = (size_t)(p->desc.max_hits > 0 ? p->desc.max_hits : 1) + 4, me = (size_t)p->desc.max_events;
+        HCK(cudaStreamCreateWithFlags(&p->h_stream, cudaStreamNonBlocking));
+        HCK(cudaMalloc((void**)&p->hd_u, mh * 4));
+        HCK(cudaMalloc((void**)&p->hd_v, mh * 4));
+        HCK(cudaMalloc((void**)&p->hd_off, (me + 1) * 8));
+        HCK(cudaMalloc((void**)&p->hd_cands, me * p->desc.max_candidates * sizeof(Candidate)));
+        HCK(cudaMalloc((void**)&p->hd_nfound, me * 4));
+        HCK(cudaMalloc((void**)&p->hd_labels, mh * 4));
+    }
+    cudaStream_t st = p->h_stream;
+    HCK(cudaMemcpyAsync(p->hd_off, h_offsets, (size_t)(n_events + 1) * 8, cudaMemcpyHostToDevice, st));
+    if (n_hits > 0) {
+        HCK(cudaMemcpyAsync(p->hd_u, h_u, (size_t)n_hits * 4, cudaMemcpyHostToDevice, st));
+        HCK(cudaMemcpyAsync(p->hd_v, h_v, (size_t)n_hits * 4, cudaMemcpyHostToDevice, st));
+    }
+    int rc = hough_find_clusters(p, p->hd_u, p->hd_v, reinterpret_cast<const int64_t*>(p->hd_off), n_events,
+                                 reinterpret_cast<hough_candidate_t*>(p->hd_cands), p->hd_nfound, st);
+    if (rc) return rc;
+    if (h_labels) {
+        rc = hough_assign_hits(p, p->hd_u, p->hd_v, reinterpret_cast<const int64_t*>(p->hd_off), n_events,
+                               reinterpret_cast<const hough_candidate_t*>(p->hd_cands), p->hd_nfound, p->hd_labels, st);
+        if (rc) return rc;
+        if (n_hits > 0) HCK(cudaMemcpyAsync(h_labels, p->hd_labels, (size_t)n_hits * 4, cudaMemcpyDeviceToHost, st));
+    }
+    if (h_cands) HCK(cudaMemcpyAsync(h_cands, p->hd_cands, (size_t)n_events * p->desc.max_candidates * sizeof(Candidate), cudaMemcpyDeviceToHost, st));
+    if (h_n_found) HCK(cudaMemcpyAsync(h_n_found, p->hd_nfound, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st));
+    HCK(cudaStreamSynchronize(st));
+    return HOUGH_OK;
+}
+
+int hough_measure_smem_atomic_peak(int32_t device, double millis, double* ops_per_s, double* sm_clock_mhz)
+{
+    if (!ops_per_s || device < 0 || !(millis > 0)) return HOUGH_EINVAL;
+    HCK(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    HCK(cudaGetDeviceProperties(&prop, device));
+    const int threads = 1024, cps = 2, rows = 256;
+    const int grid = prop.multiProcessorCount * cps;
+    const size_t sm = (size_t)rows * 128;
+    unsigned long long* d_cyc = nullptr;
+    uint32_t* d_sink = nullptr;
+    HCK(cudaMalloc((void**)&d_cyc, (size_t)grid * 8));
+    HCK(cudaMalloc((void**)&d_sink, 4));
+    cudaEvent_t e0, e1;
+    HCK(cudaEventCreate(&e0));
+    HCK(cudaEventCreate(&e1));
+    int iters = 2000;
+    float ms = 0;
+    for (int pass = 0; pass < 3; ++pass) {  // warm-up, calibration, measurement
+        HCK(cudaEventRecord(e0));
+        hough::smem_atomic_peak_kernel<<<grid, threads, sm>>>(iters, rows, d_cyc, d_sink);
+        HCK(cudaGetLastError());
+        HCK(cudaEventRecord(e1));
+        HCK(cudaEventSynchronize(e1));
+        HCK(cudaEventElapsedTime(&ms, e0, e1));
+        if (pass == 1) {
+            double want = iters * (millis / (ms > 1e-3 ? ms : 1e-3));
+            iters = want > 5e7 ? 50000000 : (want < 100 ? 100 : (int)want);
+        }
+    }
+    std::vector<unsigned long long> cyc(grid);
+    HCK(cudaMemcpy(cyc.data(), d_cyc, (size_t)grid * 8, cudaMemcpyDeviceToHost));
+    double avg = 0;
+    for (int i = 0; i < grid; ++i) avg += (double)cyc[i];
+    avg /= grid;
+    *ops_per_s = (double)iters * 8.0 * threads * grid / (ms * 1e-3);
+    if (sm_clock_mhz) *sm_clock_mhz = avg / (ms * 1e-3) / 1e6;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d_cyc); cudaFree(d_sink);
+    return HOUGH_OK;
+}
+
+}  // extern "C"
