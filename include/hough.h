@@ -93,6 +93,10 @@ typedef struct {
     int32_t counter_bytes;                 /* width of the shared-memory counters (2 or 4)                  */
     int32_t threads_per_cta, ctas_per_sm, n_ctas, smem_bytes_per_cta;
     int32_t n_sm;
+    /* fast kernel (0 in all fields when the plan cannot use it): column groups per tile row, launch shape and the
+     * per-event capacities beyond which an event is left to the general kernel */
+    int32_t fast_groups, fast_threads, fast_ctas, fast_smem_bytes;
+    int32_t fast_hits_cap, fast_on_cap, fast_peak_cap, fast_strip_list_cap;
 } hough_plan_info_t;
 
 /* Validate the descriptor, derive F, build the int32 cos/sin tables C_q[t] = llround(cos(theta_t) M),
@@ -142,6 +146,11 @@ int hough_plan_status(hough_plan_t* plan, int32_t* out, void* stream);
 
 /* Number of kernels the library has launched through this plan since creation. */
 int64_t hough_plan_launch_count(const hough_plan_t* plan);
+
+/* Diagnostic: reads and clears 16 per-phase SM-cycle sums (summed over CTAs) that the event kernel keeps only when
+ * the library is built with -DHOUGH_PHASE_TIMERS; all zeros otherwise.  h_out16[15] is always the number of events the
+ * last hough_find_clusters call on this plan handed from the fast kernel to the general kernel.  Synchronises `stream`. */
+int hough_plan_debug_counters(hough_plan_t* plan, uint64_t* h_out16, void* stream);
 
 /* Measures the conflict-free shared-memory atomic-add rate of the device (the roofline denominator of the
  * vote kernel): every SM runs `red.shared.add.u32` with lane = bank for about `millis` ms.

@@ -13,7 +13,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 SOURCES = [os.path.join(_HERE, "csrc", "hough_lib.cu")]
-DEPENDS = SOURCES + [os.path.join(_HERE, "csrc", "hough_kernels.cuh"), os.path.join(_ROOT, "include", "hough.h")]
+DEPENDS = SOURCES + [os.path.join(_HERE, "csrc", "hough_kernels.cuh"), os.path.join(_HERE, "csrc", "hough_fast.cuh"), os.path.join(_ROOT, "include", "hough.h")]
 LIB = os.path.join(_HERE, "libhough.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math",
@@ -38,7 +38,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+    extra = os.environ.get("HOUGH_NVCC_EXTRA", "").split()      # e.g. -DHOUGH_PHASE_TIMERS for the diagnostic build
+    cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

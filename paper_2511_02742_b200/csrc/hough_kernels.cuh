@@ -16,6 +16,17 @@
 
 namespace hough {
 
+// Per-phase SM-cycle sums (diagnostic build only: -DHOUGH_PHASE_TIMERS); read back with hough_plan_debug_counters.
+#ifdef HOUGH_PHASE_TIMERS
+#define HOUGH_PT(k)                                                                     \
+    do {                                                                                \
+        __syncthreads();                                                                \
+        if (threadIdx.x == 0) { const long long now_ = clock64(); pt_acc[k] += now_ - pt_last; pt_last = now_; } \
+    } while (0)
+#else
+#define HOUGH_PT(k) do { } while (0)
+#endif
+
 constexpr int kLBits = 22;                       // linear bin index L = t * n_rho + r < 2^22
 constexpr uint32_t kLMask = (1u << kLBits) - 1;  // union-find words: epoch tag (10 bits) | L
 constexpr uint32_t kEpochMax = (1u << (32 - kLBits)) - 1;
@@ -42,6 +53,21 @@ struct DevParams {
     uint32_t* epoch;    // [n_ctas]
     int* status;
     unsigned int* work_counter;
+    unsigned long long* phase_cycles;  // [16] diagnostic counters
+    // ---- fast path (hough_fast.cuh); f_enabled == 0 when the plan cannot use it
+    int f_enabled;
+    int rho_shift;                   // log2(n_rho) if n_rho is a power of two, else -1
+    int fk, fsh;                     // log2(row bytes), F - fk
+    int fS, f_nstrips, f_tile_bytes; // theta rows per strip (64 G), strips per event
+    int fHB, fSLCAP, fPCAP, fnsbits; // staged hits, strip list, peak list, log2(hash slots)
+    int f_oncap;                     // on bins an event may have on the fast path (3/4 of the hash slots)
+    int f_off_hits, f_off_halo, f_off_slist, f_off_peaks, f_off_hist, f_off_kept;
+    const int* fCq;                  // [f_nstrips * fS], zero padded
+    const int* fSq;
+    uint32_t* f_onlist;              // [n_fast_ctas][f_oncap] linear indices of the on bins of the current event
+    int* deferred;                   // [max_events] events the fast kernel left to the general kernel
+    unsigned int* deferred_count;
+    unsigned int* f_work_counter;
 };
 
 struct Candidate {  // mirrors hough_candidate_t
@@ -95,9 +121,10 @@ __device__ __forceinline__ void uf_union(uint32_t* parent, uint32_t a, uint32_t 
 // ---------------------------------------------------------------- S0: staging
 
 struct StageCtx {
-    int2* hits;   // [HB]: safe hits from the front, unsafe hits from the back
+    int2* hits;   // [hb]: safe hits from the front, unsafe hits from the back
     int* n_safe;  // shared counters
     int* n_unsafe;
+    int hb;
 };
 
 __device__ __forceinline__ void stage_one(const DevParams& P, const StageCtx& sc, float u, float v)
@@ -110,7 +137,7 @@ __device__ __forceinline__ void stage_one(const DevParams& P, const StageCtx& sc
     if (P.safe_enabled && r2 <= P.r2safe) {
         sc.hits[atomicAdd(sc.n_safe, 1)] = make_int2(uq, vq);
     } else {
-        sc.hits[P.HB - 1 - atomicAdd(sc.n_unsafe, 1)] = make_int2(uq, vq);
+        sc.hits[sc.hb - 1 - atomicAdd(sc.n_unsafe, 1)] = make_int2(uq, vq);
     }
 }
 
@@ -219,8 +246,11 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
 hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* __restrict__ v,
                    const long long* __restrict__ offsets, int n_events, Candidate* __restrict__ cands,
                    int* __restrict__ n_found, void* __restrict__ acc_out, int acc_is_u16,
-                   unsigned long long* __restrict__ digest_out)
+                   unsigned long long* __restrict__ digest_out, const int* __restrict__ event_list,
+                   const unsigned int* __restrict__ event_list_count)
 {
+    // with an event list, the kernel processes events event_list[0 .. *event_list_count) instead of 0 .. n_events
+    if (event_list) n_events = (int)*event_list_count;
     constexpr int TPW = 4 / CW;
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ EventShared sh;
@@ -235,13 +265,17 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
     const uint32_t colbase = smem_addr(tile) + 4u * lane;
-    const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe};
+    const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe, P.HB};
 
     uint32_t* parent = P.parent + (size_t)blockIdx.x * P.n_bins;
     uint32_t* csize = P.csize + (size_t)blockIdx.x * P.n_bins;
     uint2* onlist = P.onlist + (size_t)blockIdx.x * P.n_bins;
     uint2* peaks_ovf = P.peaks_ovf + (size_t)blockIdx.x * (P.n_bins / 4 + 1);
     uint32_t epoch = DUMP ? 0 : P.epoch[blockIdx.x];
+#ifdef HOUGH_PHASE_TIMERS
+    long long pt_acc[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    long long pt_last = clock64();
+#endif
 
     while (true) {
         __syncthreads();  // previous event fully done (also protects sh.event)
@@ -255,8 +289,8 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
             sh.digest = 0;
         }
         __syncthreads();
-        const int e = sh.event;
-        if (e >= n_events) break;
+        if (sh.event >= n_events) break;
+        const int e = event_list ? event_list[sh.event] : sh.event;
 
         const long long g0 = offsets[e], g1 = offsets[e + 1];
         long long ne64 = g1 - g0;
@@ -278,6 +312,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
         }
 
         const int n_strips_e = (DUMP || ne > 0) ? P.n_strips : 0;  // an empty event has no on bins
+        HOUGH_PT(0);
         for (int strip = 0; strip < n_strips_e; ++strip) {
             const int base = strip * P.S;  // first theta row of the strip
             const bool last_strip = (strip == P.n_strips - 1);
@@ -300,6 +335,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
                     Sn[g][j] = __ldg(P.Sq + base + tl);
                     O[g][j] = (base + tl < P.n_theta) ? P.Oq : -(1 << P.F);
                 }
+            HOUGH_PT(1);
 
             for (int chunk = 0; chunk < n_chunks; ++chunk) {
                 if (n_chunks > 1 || strip == 0) {
@@ -310,12 +346,14 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
                     stage_hits(P, sc, u, v, g0 + (long long)chunk * P.HB, cn);
                 }
                 __syncthreads();  // tile zeroed, hits staged
+                HOUGH_PT(2);
                 const int ns = sh.n_safe, nu = sh.n_unsafe;
                 if (full) vote_hits<CW, G, false>(P, hits, 0, ns, colbase, C, Sn, O);
                 else vote_hits<CW, G, true>(P, hits, 0, ns, colbase, C, Sn, O);
                 vote_hits<CW, G, true>(P, hits, P.HB - nu, nu, colbase, C, Sn, O);
             }
             __syncthreads();  // all votes of the strip are in
+            HOUGH_PT(3);
 
             if (DUMP) {
                 // materialise the strip: acc_out[e][t][r], theta-major; digest over non-zero bins
@@ -385,6 +423,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
                 }
             }
             __syncthreads();
+            HOUGH_PT(4);
             if (!last_strip) {  // keep the last two theta rows for the next strip's tests
                 for (int r = tid; r < P.n_rho; r += nthr) {
                     halo[r] = tile_get<CW>(tile, P.S, r, P.S - 2);
@@ -392,6 +431,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
                 }
             }
             __syncthreads();
+            HOUGH_PT(5);
         }  // strips
 
         if (DUMP) {
@@ -416,11 +456,13 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
             }
         }
         __syncthreads();
+        HOUGH_PT(6);
         for (int i = tid; i < n_on; i += nthr) {
             const uint32_t L = __ldcg(onlist + i).x;
             atomicAdd(csize + uf_find(parent, L, tag), 1u);
         }
         __threadfence();
+        HOUGH_PT(7);
 
         // ---------------- S4: rank the peaks by key = (~votes, L) ascending, keep the first K
         auto peak_key = [&](int i) -> unsigned long long {
@@ -476,6 +518,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
         } else {
             __syncthreads();
         }
+        HOUGH_PT(8);
         for (int i = tid; i < n_pk; i += nthr) {
             const unsigned long long k = peak_key(i);
             if (k <= kth) kept[atomicAdd(&sh.n_kept, 1)] = k;
@@ -514,8 +557,13 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
             dst[1] = make_int4(cd.cluster_nbins, __float_as_int(cd.theta), __float_as_int(cd.rho), 0);
         }
         if (tid == 0) n_found[e] = n_pk;
+        HOUGH_PT(9);
     }
     if (!DUMP && threadIdx.x == 0) P.epoch[blockIdx.x] = epoch;
+#ifdef HOUGH_PHASE_TIMERS
+    if (threadIdx.x == 0)
+        for (int k = 0; k < 12; ++k) atomicAdd(P.phase_cycles + k, (unsigned long long)pt_acc[k]);
+#endif
 }
 
 // ---------------------------------------------------------------- S5: assignment

@@ -3,6 +3,7 @@
 // No torch, no Python: plain CUDA runtime.  Built for sm_100a only (see paper_2511_02742_b200/build.py).
 #include "../../include/hough.h"
 #include "hough_kernels.cuh"
+#include "hough_fast.cuh"
 
 #include <math.h>
 #include <stdio.h>
@@ -41,6 +42,12 @@ struct hough_plan {
     int n_ctas, threads, smem_bytes;
     int assign_ctas;
     int64_t launches;
+    // fast path (hough_fast.cuh)
+    int f_G, f_maxt, f_minb, f_threads, f_ctas, f_smem;
+    int* d_fcos;
+    int* d_fsin;
+    uint32_t* d_fonlist;
+    int* d_deferred;
     // owned device memory
     int* d_cos;
     int* d_sin;
@@ -86,23 +93,25 @@ static SmemLayout layout_smem(int tile_bytes, int HB, int n_rho, int PCAP, int K
 template <int CW, int G, bool DUMP>
 static cudaError_t launch_event_kernel(const hough_plan* p, const float* u, const float* v, const long long* off, int n_events,
                                        Candidate* cands, int* n_found, void* acc, int acc_u16, unsigned long long* digest,
-                                       cudaStream_t st)
+                                       cudaStream_t st, const int* elist, const unsigned int* ecount)
 {
     auto k = hough::hough_event_kernel<CW, G, DUMP>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes);
     if (e != cudaSuccess) return e;
-    k<<<p->n_ctas, p->threads, p->smem_bytes, st>>>(p->P, u, v, off, n_events, cands, n_found, acc, acc_u16, digest);
+    e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    k<<<p->n_ctas, p->threads, p->smem_bytes, st>>>(p->P, u, v, off, n_events, cands, n_found, acc, acc_u16, digest, elist, ecount);
     return cudaGetLastError();
 }
 
 template <bool DUMP>
 static cudaError_t dispatch_event_kernel(const hough_plan* p, const float* u, const float* v, const long long* off, int n_events,
                                          Candidate* cands, int* n_found, void* acc, int acc_u16, unsigned long long* digest,
-                                         cudaStream_t st)
+                                         cudaStream_t st, const int* elist = nullptr, const unsigned int* ecount = nullptr)
 {
 #define HOUGH_CASE(CW_, G_)                                                                                                 \
     if (p->cw == CW_ && p->G == G_)                                                                                         \
-        return launch_event_kernel<CW_, G_, DUMP>(p, u, v, off, n_events, cands, n_found, acc, acc_u16, digest, st);
+        return launch_event_kernel<CW_, G_, DUMP>(p, u, v, off, n_events, cands, n_found, acc, acc_u16, digest, st, elist, ecount);
     HOUGH_CASE(2, 1) HOUGH_CASE(2, 2) HOUGH_CASE(2, 3) HOUGH_CASE(2, 4) HOUGH_CASE(2, 6) HOUGH_CASE(2, 8)
     HOUGH_CASE(4, 1) HOUGH_CASE(4, 2) HOUGH_CASE(4, 3) HOUGH_CASE(4, 4) HOUGH_CASE(4, 6) HOUGH_CASE(4, 8)
 #undef HOUGH_CASE
@@ -110,6 +119,66 @@ static cudaError_t dispatch_event_kernel(const hough_plan* p, const float* u, co
 }
 
 static const int kGroupChoices[] = {8, 6, 4, 3, 2, 1};
+
+// ---- fast kernel: instantiations (G, max threads, min CTAs per SM) and their launch
+template <int G, int MAXT, int MINB>
+static cudaError_t launch_fast(const hough_plan* p, const float* u, const float* v, const long long* off, int n_events,
+                               Candidate* cands, int* n_found, cudaStream_t st)
+{
+    auto k = hough::hough_fast_kernel<G, MAXT, MINB>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, p->f_smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    if (getenv("HOUGH_DEBUG_OCCUPANCY")) {
+        int occ = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, p->f_threads, p->f_smem);
+        cudaFuncAttributes fa;
+        cudaFuncGetAttributes(&fa, k);
+        cudaDeviceProp prop;
+        cudaGetDeviceProperties(&prop, p->desc.device);
+        fprintf(stderr, "hough_fast_kernel<%d,%d,%d>: %d threads, %d B dynamic smem -> %d CTAs/SM (regs %d, static smem %zu, local %zu; SM smem %zu, "
+                        "reserved/block %zu, regs/SM %d)\n", G, MAXT, MINB, p->f_threads, p->f_smem, occ, fa.numRegs, fa.sharedSizeBytes,
+                fa.localSizeBytes, prop.sharedMemPerMultiprocessor, prop.reservedSharedMemPerBlock, prop.regsPerMultiprocessor);
+        for (int sm = p->f_smem; sm > p->f_smem - 8192; sm -= 512) {
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, p->f_threads, sm);
+            if (occ >= 2) { fprintf(stderr, "  2 CTAs/SM fit at %d B dynamic smem\n", sm); break; }
+        }
+    }
+    k<<<p->f_ctas, p->f_threads, p->f_smem, st>>>(p->P, u, v, off, n_events, cands, n_found);
+    return cudaGetLastError();
+}
+
+static cudaError_t dispatch_fast(const hough_plan* p, const float* u, const float* v, const long long* off, int n_events,
+                                 Candidate* cands, int* n_found, cudaStream_t st)
+{
+#define HOUGH_FCASE(G_, T_, B_)                                                                   \
+    if (p->f_G == G_ && p->f_maxt == T_ && p->f_minb == B_) return launch_fast<G_, T_, B_>(p, u, v, off, n_events, cands, n_found, st);
+    HOUGH_FCASE(1, 768, 2) HOUGH_FCASE(2, 768, 2) HOUGH_FCASE(4, 768, 2)
+    HOUGH_FCASE(1, 1024, 2) HOUGH_FCASE(2, 1024, 2) HOUGH_FCASE(4, 1024, 2)
+    HOUGH_FCASE(1, 1024, 1) HOUGH_FCASE(2, 1024, 1) HOUGH_FCASE(4, 1024, 1)
+    HOUGH_FCASE(1, 512, 3) HOUGH_FCASE(2, 512, 3)
+#undef HOUGH_FCASE
+    return cudaErrorInvalidValue;
+}
+
+struct FastLayout {
+    int off_hits, off_halo, off_slist, off_peaks, off_hist, off_kept, total;
+};
+static FastLayout layout_fast(int tile_bytes, int HB, int n_rho, int SLCAP, int PCAP, int K)
+{
+    FastLayout L;
+    size_t o = align_up((size_t)tile_bytes, 16);
+    L.off_hits = (int)o;   o = align_up(o + (size_t)HB * 8, 16);
+    L.off_halo = (int)o;   o = align_up(o + (size_t)2 * n_rho * 2, 16);
+    L.off_slist = (int)o;  o = align_up(o + (size_t)SLCAP * 4, 16);
+    L.off_peaks = (int)o;  o = align_up(o + (size_t)PCAP * 4, 16);
+    L.off_hist = (int)o;   o = align_up(o + 256 * 4, 16);
+    L.off_kept = (int)o;   o = align_up(o + (size_t)K * 16, 16);
+    o += 64;               // FastShared control block
+    L.total = (int)o;
+    return L;
+}
 
 extern "C" {
 
@@ -246,6 +315,47 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     p->assign_ctas = n_sm * 8;
     p->launches = 0;
 
+    // ---- fast kernel configuration (hough_fast.cuh): u16 counters, rows of 128 G bytes, several CTAs per SM
+    p->f_G = 0;
+    FastLayout flay{};
+    int f_S = 0, f_nstrips = 0, f_tile = 0, f_HB = 0, f_SLCAP = 0, f_PCAP = 0, f_nsbits = 0, f_k = 0;
+    if (cw == 2 && d->vote_threshold <= 1023 && K <= 1000 && d->max_hits_per_event >= 1 && !env_int("HOUGH_NO_FAST", 0)) {
+        struct Cand { int G, maxt, minb, threads, cps; };
+        // preference order: two co-resident CTAs (overlap of vote and scan/cluster phases), widest rows first
+        const Cand cands[] = {{4, 768, 2, 768, 2}, {2, 768, 2, 768, 2}, {1, 768, 2, 768, 2}, {4, 1024, 1, 1024, 1}, {2, 1024, 1, 1024, 1}, {1, 1024, 1, 1024, 1}};
+        const int want_G = env_int("HOUGH_FAST_G", 0), want_t = env_int("HOUGH_FAST_MAXT", 0), want_b = env_int("HOUGH_FAST_MINB", 0);
+        const int want_threads = env_int("HOUGH_FAST_THREADS", 0);
+        std::vector<Cand> list(cands, cands + sizeof(cands) / sizeof(cands[0]));
+        if (want_G && want_t && want_b) list.assign(1, Cand{want_G, want_t, want_b, want_threads > 0 ? want_threads : want_t, want_b});
+        for (const Cand& c : list) {
+            const int rows = 64 * c.G;
+            if (rows > 64 && rows / 2 >= d->n_theta) continue;  // a narrower tile already covers every theta row
+            int kk = 7; while ((128 << (kk - 7)) < 128 * c.G) ++kk;
+            const int sh = F - kk;
+            if (sh < 0) continue;
+            // unsigned range of a' = a + (tile_base << sh): tile_base < 4096 (static shared memory + alignment)
+            if (((unsigned long long)4096 << sh) + ((unsigned long long)d->n_rho << F) > 0xffffffffull) continue;
+            const int budget = (c.cps == 1 ? smem_optin : (smem_sm / c.cps - reserved)) - 128;  // the kernel has no static shared memory
+            const int lim = budget < smem_optin ? budget : smem_optin;
+            const int tile = d->n_rho * 128 * c.G;
+            int hb = (int)align_up((size_t)(d->max_hits_per_event < 32 ? 32 : d->max_hits_per_event), 32);
+            if (hb > 8192) hb = 8192;
+            int slcap = env_int("HOUGH_FAST_SLCAP", 2048), pcap = env_int("HOUGH_FAST_PCAP", 4096);
+            while (layout_fast(tile, hb, d->n_rho, slcap, pcap, K).total > lim && pcap > 2048) pcap -= 256;
+            while (layout_fast(tile, hb, d->n_rho, slcap, pcap, K).total > lim && slcap > 1024) slcap -= 256;
+            while (layout_fast(tile, hb, d->n_rho, slcap, pcap, K).total > lim && hb > 1024) hb -= 32;
+            const FastLayout L = layout_fast(tile, hb, d->n_rho, slcap, pcap, K);
+            if (L.total > lim) continue;
+            int nsb = 16;
+            while (nsb > 8 && (size_t)6 << nsb > (size_t)L.off_kept) --nsb;
+            if ((size_t)6 << nsb > (size_t)L.off_kept) continue;
+            p->f_G = c.G; p->f_maxt = c.maxt; p->f_minb = c.minb; p->f_threads = c.threads; p->f_ctas = n_sm * c.cps; p->f_smem = L.total;
+            flay = L; f_S = rows; f_nstrips = (d->n_theta + rows - 1) / rows; f_tile = tile; f_HB = hb; f_SLCAP = slcap; f_PCAP = pcap;
+            f_nsbits = nsb; f_k = kk;
+            break;
+        }
+    }
+
     // ---- device memory
     const size_t n_bins = (size_t)d->n_theta * d->n_rho;
     const size_t tab = (size_t)n_strips * S;
@@ -263,6 +373,19 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     ok = ok && (ce = cudaMemcpy(p->d_sin, pads.data(), tab * 4, cudaMemcpyHostToDevice)) == cudaSuccess;
     ok = ok && (ce = cudaMemset(p->d_scratch, 0, scratch_bytes)) == cudaSuccess;
     ok = ok && (ce = cudaMemset(p->d_status, 0, 256)) == cudaSuccess;
+    const int f_oncap = p->f_G ? (3 << f_nsbits) / 4 : 0;
+    if (p->f_G) {
+        const size_t ftab = (size_t)f_nstrips * f_S;
+        std::vector<int32_t> fc(ftab, 0), fs(ftab, 0);
+        memcpy(fc.data(), p->h_cos.data(), sizeof(int32_t) * d->n_theta);
+        memcpy(fs.data(), p->h_sin.data(), sizeof(int32_t) * d->n_theta);
+        ok = ok && (ce = cudaMalloc((void**)&p->d_fcos, ftab * 4)) == cudaSuccess;
+        ok = ok && (ce = cudaMalloc((void**)&p->d_fsin, ftab * 4)) == cudaSuccess;
+        ok = ok && (ce = cudaMalloc((void**)&p->d_fonlist, (size_t)p->f_ctas * f_oncap * 4)) == cudaSuccess;
+        ok = ok && (ce = cudaMalloc((void**)&p->d_deferred, (size_t)d->max_events * 4)) == cudaSuccess;
+        ok = ok && (ce = cudaMemcpy(p->d_fcos, fc.data(), ftab * 4, cudaMemcpyHostToDevice)) == cudaSuccess;
+        ok = ok && (ce = cudaMemcpy(p->d_fsin, fs.data(), ftab * 4, cudaMemcpyHostToDevice)) == cudaSuccess;
+    }
     if (!ok) {
         const int rc = (ce == cudaErrorMemoryAllocation) ? HOUGH_ENOMEM : cuda_fail(ce, "plan allocation");
         (void)cudaGetLastError();
@@ -310,12 +433,28 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     }
     P.status = p->d_status;
     P.work_counter = p->d_counter;
+    P.f_work_counter = p->d_counter + 1;
+    P.deferred_count = p->d_counter + 2;
+    P.f_enabled = p->f_G != 0;
+    P.rho_shift = -1;
+    for (int b = 0; b < 31; ++b) if ((1 << b) == d->n_rho) P.rho_shift = b;
+    if (p->f_G) {
+        P.fk = f_k; P.fsh = F - f_k; P.fS = f_S; P.f_nstrips = f_nstrips; P.f_tile_bytes = f_tile;
+        P.fHB = f_HB; P.fSLCAP = f_SLCAP; P.fPCAP = f_PCAP; P.fnsbits = f_nsbits; P.f_oncap = f_oncap;
+        P.f_off_hits = flay.off_hits; P.f_off_halo = flay.off_halo; P.f_off_slist = flay.off_slist;
+        P.f_off_peaks = flay.off_peaks; P.f_off_hist = flay.off_hist; P.f_off_kept = flay.off_kept;
+        P.fCq = p->d_fcos; P.fSq = p->d_fsin; P.f_onlist = p->d_fonlist; P.deferred = p->d_deferred;
+    }
+    P.phase_cycles = reinterpret_cast<unsigned long long*>(p->d_status) + 16;  // bytes 128..255 of the status block
 
     hough_plan_info_t& I = p->info;
     I.hit_frac_bits = H; I.acc_frac_bits = F; I.rho_offset_q = (int32_t)Oq; I.assign_window_q = (int32_t)Wq;
     I.strip_rows = S; I.n_strips = n_strips; I.counter_bytes = cw;
     I.threads_per_cta = threads; I.ctas_per_sm = ctas_per_sm; I.n_ctas = p->n_ctas; I.smem_bytes_per_cta = lay.total;
     I.n_sm = n_sm;
+    I.fast_groups = p->f_G; I.fast_threads = p->f_G ? p->f_threads : 0; I.fast_ctas = p->f_G ? p->f_ctas : 0;
+    I.fast_smem_bytes = p->f_G ? p->f_smem : 0; I.fast_hits_cap = f_HB; I.fast_on_cap = f_oncap; I.fast_peak_cap = f_PCAP;
+    I.fast_strip_list_cap = f_SLCAP;
     *out = p;
     return HOUGH_OK;
 }
@@ -326,6 +465,7 @@ int hough_plan_destroy(hough_plan_t* p)
     (void)cudaSetDevice(p->desc.device);
     (void)cudaDeviceSynchronize();
     cudaFree(p->d_cos); cudaFree(p->d_sin); cudaFree(p->d_scratch); cudaFree(p->d_status);
+    cudaFree(p->d_fcos); cudaFree(p->d_fsin); cudaFree(p->d_fonlist); cudaFree(p->d_deferred);
     cudaFree(p->hd_u); cudaFree(p->hd_v); cudaFree(p->hd_off); cudaFree(p->hd_cands); cudaFree(p->hd_nfound); cudaFree(p->hd_labels);
     if (p->h_stream) cudaStreamDestroy(p->h_stream);
     (void)cudaGetLastError();
@@ -343,6 +483,20 @@ int hough_plan_query(const hough_plan_t* p, hough_plan_info_t* info, int32_t* h_
 }
 
 int64_t hough_plan_launch_count(const hough_plan_t* p) { return p ? p->launches : 0; }
+
+int hough_plan_debug_counters(hough_plan_t* p, uint64_t* h_out16, void* stream)
+{
+    if (!p || !h_out16) return HOUGH_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(p->desc.device));
+    HCK(cudaMemcpyAsync(h_out16, p->P.phase_cycles, 16 * sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+    HCK(cudaMemsetAsync(p->P.phase_cycles, 0, 16 * sizeof(uint64_t), st));
+    unsigned int deferred = 0;  // events the last hough_find_clusters call left to the general kernel
+    HCK(cudaMemcpyAsync(&deferred, p->P.deferred_count, sizeof deferred, cudaMemcpyDeviceToHost, st));
+    HCK(cudaStreamSynchronize(st));
+    h_out16[15] = deferred;
+    return HOUGH_OK;
+}
 
 int hough_plan_status(hough_plan_t* p, int32_t* out, void* stream)
 {
@@ -389,7 +543,17 @@ int hough_find_clusters(hough_plan_t* p, const float* d_u, const float* d_v, con
     if (n_events == 0) return HOUGH_OK;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     HCK(cudaSetDevice(p->desc.device));
-    HCK(cudaMemsetAsync(p->d_counter, 0, sizeof(unsigned int), st));
+    HCK(cudaMemsetAsync(p->d_counter, 0, 4 * sizeof(unsigned int), st));
+    if (p->f_G) {
+        // fast kernel first; the events it could not take (list in d_deferred) go through the general kernel
+        HCK(dispatch_fast(p, d_u, d_v, reinterpret_cast<const long long*>(d_offsets), n_events, reinterpret_cast<Candidate*>(d_cands),
+                          d_n_found, st));
+        HCK(dispatch_event_kernel<false>(p, d_u, d_v, reinterpret_cast<const long long*>(d_offsets), n_events,
+                                         reinterpret_cast<Candidate*>(d_cands), d_n_found, nullptr, 0, nullptr, st, p->d_deferred,
+                                         p->P.deferred_count));
+        p->launches += 2;
+        return HOUGH_OK;
+    }
     HCK(dispatch_event_kernel<false>(p, d_u, d_v, reinterpret_cast<const long long*>(d_offsets), n_events,
                                      reinterpret_cast<Candidate*>(d_cands), d_n_found, nullptr, 0, nullptr, st));
     p->launches += 1;

@@ -31,7 +31,7 @@ CANDIDATE_DTYPE = np.dtype([("theta_bin", "<i4"), ("rho_bin", "<i4"), ("votes", 
 CANDIDATE_WORDS = 8   # a record is 8 x 32-bit words; device tensors of records are int32 [E, K, 8]
 
 EXPORTS = ("hough_plan_create", "hough_plan_destroy", "hough_vote", "hough_find_clusters", "hough_assign_hits",
-           "hough_run_host", "hough_plan_query", "hough_plan_status", "hough_plan_launch_count",
+           "hough_run_host", "hough_plan_query", "hough_plan_status", "hough_plan_launch_count", "hough_plan_debug_counters",
            "hough_measure_smem_atomic_peak", "hough_strerror", "hough_last_cuda_error", "hough_version")
 
 
@@ -47,7 +47,9 @@ class hough_plan_desc_t(ctypes.Structure):
 class hough_plan_info_t(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in ("hit_frac_bits", "acc_frac_bits", "rho_offset_q", "assign_window_q",
                                               "strip_rows", "n_strips", "counter_bytes", "threads_per_cta", "ctas_per_sm",
-                                              "n_ctas", "smem_bytes_per_cta", "n_sm")]
+                                              "n_ctas", "smem_bytes_per_cta", "n_sm", "fast_groups", "fast_threads",
+                                              "fast_ctas", "fast_smem_bytes", "fast_hits_cap", "fast_on_cap", "fast_peak_cap",
+                                              "fast_strip_list_cap")]
 
 
 class HoughError(RuntimeError):
@@ -83,6 +85,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     L.hough_plan_status.argtypes = [vp, ctypes.POINTER(i32), vp]
     L.hough_plan_launch_count.argtypes = [vp]
     L.hough_plan_launch_count.restype = i64
+    L.hough_plan_debug_counters.argtypes = [vp, vp, vp]
     L.hough_measure_smem_atomic_peak.argtypes = [i32, ctypes.c_double, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.hough_strerror.argtypes = [ctypes.c_int]
     L.hough_strerror.restype = ctypes.c_char_p
@@ -151,6 +154,14 @@ def hough_plan_status(plan: Plan, stream: Optional[torch.cuda.Stream] = None) ->
 
 def hough_plan_launch_count(plan: Plan) -> int:
     return int(load_library().hough_plan_launch_count(plan.handle))
+
+
+def hough_plan_debug_counters(plan: Plan, stream=None) -> np.ndarray:
+    """uint64 [16] per-phase SM-cycle sums (zeros unless libhough was built with -DHOUGH_PHASE_TIMERS); clears them."""
+    out = np.zeros(16, np.uint64)
+    _check(load_library().hough_plan_debug_counters(plan.handle, out.ctypes.data, _stream_ptr(plan, stream)),
+           "hough_plan_debug_counters")
+    return out
 
 
 def _stream_ptr(plan: Plan, stream) -> ctypes.c_void_p:
