@@ -2,28 +2,30 @@
 //
 // Same results as hough_event_kernel (hough_kernels.cuh), for the common case only; an event that does not fit the
 // fast path's capacities is appended to a "deferred" list and processed afterwards by the general kernel:
-//     more hits than the staged-hit buffer, a bin count above 1023, more peaks than the shared peak list,
-//     more on bins than the cluster hash table holds, more ties at the K-th vote count than the tie buffer.
+//     more hits than the staged-hit buffer, a bin count above 1023, more on bins in one strip than the strip list
+//     holds, more on bins / peaks in the event than the parent / peak arrays hold, more ties at the K-th vote count
+//     than the tie buffer.
 //
-// Per event (one CTA at a time, several CTAs per SM so that one CTA's scan / cluster phases fill the issue slots the
-// other leaves while it votes):
+// Per event (one CTA at a time):
 //   S0  stage     fp32 hits -> fixed point, "safe" hits (in range for every theta) first             (O1)
 //   per strip of S = 64 G theta rows (tile [n_rho][S] of u16 counters, theta fastest, row = 128 G bytes):
 //   S1  vote      lane <-> 32-bit word column (2 theta rows), 2 IMAD + SHF + LOP3 + RED per vote:
 //                 the tile base is folded into the fixed-point offset, so ((a >> (F - k)) & ~(2^k - 1)) | column
 //                 IS the shared-memory address of the counter word                                   (Eq. 4.1)
-//   S2  scan      16-byte chunks -> compact list of on bins of the strip -> one thread per on bin:
-//                 strict-local-maximum test (1 theta row of halo kept between strips)                 (L94, L106)
-//   then, once per event, with the tile memory reused:
-//   S4a select    vote-count histogram -> threshold count -> ties ranked by index -> K best peaks
-//   S3  clusters  open-addressing hash (bin index -> slot) + union-find on the slots, 8-connectivity  (keyword L29)
-//   S4b write     32-byte records in rank order
+//   S2  scan      16-byte chunks -> compact list of the strip's on bins -> one thread per on bin:
+//                 (a) strict-local-maximum test on the counts (1 theta row of halo kept between strips) (L94, L106)
+//                 (b) the on bin's tile entry is overwritten with 0x8000 | its index in the event's on list
+//   S3  clusters  (c) each on bin reads the entries of its four earlier neighbours straight from the tile and joins
+//                 them in a union-find over on-list indices (16-bit parents in shared memory)         (keyword L29)
+//   then, once per event:
+//   S4  select    vote-count histogram -> threshold count -> ties ranked by index -> K best peaks; component sizes
+//                 of the kept peaks' components; 32-byte records in rank order
 #pragma once
 #include "hough_kernels.cuh"
 
 namespace hough {
 
-constexpr uint32_t kHashEmpty = 0xffffffffu;
+constexpr uint32_t kOnFlag = 0x8000u;  // tile entry of an on bin after step (b): kOnFlag | on-list index
 constexpr int kCountBits = 10;  // packed peak key: (1023 - votes) << 22 | L   (smaller key = better rank)
 constexpr uint32_t kCountMax = (1u << kCountBits) - 1;
 
@@ -64,21 +66,7 @@ __device__ __forceinline__ void split_L(const DevParams& P, uint32_t L, int& t, 
     else { t = (int)(L / (uint32_t)P.n_rho); r = (int)(L - (uint32_t)t * P.n_rho); }
 }
 
-__device__ __forceinline__ uint32_t hash_slot(uint32_t L, int nsbits) { return (L * 2654435761u) >> (32 - nsbits); }
-
-__device__ __forceinline__ int hash_find(const uint32_t* keys, uint32_t L, int nsbits)
-{
-    const uint32_t msk = (1u << nsbits) - 1;
-    uint32_t s = hash_slot(L, nsbits);
-    while (true) {
-        const uint32_t k = keys[s];
-        if (k == L) return (int)s;
-        if (k == kHashEmpty) return -1;
-        s = (s + 1) & msk;
-    }
-}
-
-// union-find over hash slots, 16-bit parents in shared memory (hook the larger root under the smaller one)
+// union-find over on-list indices, 16-bit parents in shared memory (hook the larger root under the smaller one)
 __device__ __forceinline__ uint32_t suf_find(volatile unsigned short* parent, uint32_t x)
 {
     uint32_t p = parent[x];
@@ -192,6 +180,15 @@ __device__ __forceinline__ bool fis_peak(const DevParams& P, const uint16_t* til
     return true;
 }
 
+
+// Tile entry of bin (strip-local theta row tl, rho bin r) after step (b): kOnFlag | on-list index for an on bin, a
+// count below the threshold otherwise.  Row -1 is the previous strip's last row (index halo); outside the grid -> 0.
+__device__ __forceinline__ uint32_t fentry_at(const DevParams& P, const uint16_t* tile, const uint16_t* ihalo_prev, int tl, int r)
+{
+    if ((unsigned)r >= (unsigned)P.n_rho) return 0;
+    return tl >= 0 ? tile[r * P.fS + tl] : ihalo_prev[r];
+}
+
 // ---------------------------------------------------------------- the fast event kernel
 
 template <int G, int MAXT, int MINB>
@@ -201,22 +198,24 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     // the control block sits at the end of the dynamic allocation: no static shared memory, so the tile starts the window
-    FastShared& sh = *reinterpret_cast<FastShared*>(smem + P.f_off_kept + (size_t)P.K * 16);
+    FastShared& sh = *reinterpret_cast<FastShared*>(smem + P.f_off_kept + (size_t)P.K * 20);
 
     uint16_t* tile = reinterpret_cast<uint16_t*>(smem);
     int2* hits = reinterpret_cast<int2*>(smem + P.f_off_hits);
-    uint16_t* halo = reinterpret_cast<uint16_t*>(smem + P.f_off_halo);
-    uint32_t* slist = reinterpret_cast<uint32_t*>(smem + P.f_off_slist);  // strip list; later the tie list
-    uint32_t* peaks = reinterpret_cast<uint32_t*>(smem + P.f_off_peaks);
-    int* hist = reinterpret_cast<int*>(smem + P.f_off_hist);              // [256] peaks per min(votes, 255)
-    uint32_t* kept = reinterpret_cast<uint32_t*>(smem + P.f_off_kept);    // [K] unordered, [K] sorted, [K] root slot, [K] size
+    uint16_t* halo = reinterpret_cast<uint16_t*>(smem + P.f_off_halo);      // [2][n_rho] counts of the previous strip's last two rows
+    uint16_t* ihalo = reinterpret_cast<uint16_t*>(smem + P.f_off_ihalo);    // [2][n_rho] entries of a strip's last row, by strip parity
+    uint32_t* slist = reinterpret_cast<uint32_t*>(smem + P.f_off_slist);    // strip list; later the tie list
+    uint32_t* peaks = reinterpret_cast<uint32_t*>(smem + P.f_off_peaks);    // [PCAP] packed keys
+    uint16_t* pidx = reinterpret_cast<uint16_t*>(smem + P.f_off_pidx);      // [PCAP] on-list index of each peak
+    unsigned short* parent = reinterpret_cast<unsigned short*>(smem + P.f_off_parent);  // [ONCAP]
+    int* hist = reinterpret_cast<int*>(smem + P.f_off_hist);                // [256] peaks per min(votes, 255)
+    uint32_t* kept = reinterpret_cast<uint32_t*>(smem + P.f_off_kept);      // [K] each: unordered keys, sorted keys, roots, sizes
     uint32_t* sorted = kept + P.K;
     uint32_t* kroot = sorted + P.K;
     uint32_t* ksize = kroot + P.K;
-    // after the last strip the memory below f_off_kept is reused: hash keys [NS] u32, then parents [NS] u16
-    uint32_t* hkeys = reinterpret_cast<uint32_t*>(smem);
-    const int NS = 1 << P.fnsbits;
-    unsigned short* hparent = reinterpret_cast<unsigned short*>(smem + (size_t)NS * 4);
+    uint16_t* kidx = reinterpret_cast<uint16_t*>(ksize + P.K);              // [K] on-list index, unordered / sorted
+    uint16_t* sidx = kidx + P.K;
+    uint16_t* roottag = tile;  // after the last strip: [ONCAP] slot + 1 of the component's best kept peak, at union-find roots
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
     const uint32_t tile_base = smem_addr(tile);
@@ -227,7 +226,6 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 #pragma unroll
     for (int g = 0; g < G; ++g) col[g] = 4u * lane + 128u * g;
     const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe, P.fHB};
-    uint32_t* onlist = P.f_onlist + (size_t)blockIdx.x * P.f_oncap;
     const uint32_t T = (uint32_t)P.T;
     const uint32_t TT = T | (T << 16);
     const int cpr = 8 * G;  // 16-byte chunks per rho row
@@ -258,15 +256,21 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             if (tid == 0) n_found[e] = 0;
             continue;
         }
-        for (int i = tid; i < P.n_rho; i += nthr) reinterpret_cast<uint32_t*>(halo)[i] = 0;  // 2 rows of u16
+        for (int i = tid; i < P.n_rho; i += nthr) {  // both count-halo rows and both index-halo rows (u16 pairs)
+            reinterpret_cast<uint32_t*>(halo)[i] = 0;
+            reinterpret_cast<uint32_t*>(ihalo)[i] = 0;
+        }
         for (int i = tid; i < 256; i += nthr) hist[i] = 0;
         stage_hits(P, sc, u, v, g0, ne);
         HOUGH_PT(0);
 
+        bool give_up = false;
         for (int strip = 0; strip < P.f_nstrips; ++strip) {
             const int base = strip * S;  // first theta row of the strip
             const bool last_strip = (strip == P.f_nstrips - 1);
             const bool full = base + S <= P.n_theta;
+            const uint16_t* ihalo_prev = ihalo + ((strip + 1) & 1) * P.n_rho;  // written by the previous strip
+            uint16_t* ihalo_cur = ihalo + (strip & 1) * P.n_rho;
             {
                 uint4* t4 = reinterpret_cast<uint4*>(tile);
                 const int n16 = P.f_tile_bytes >> 4;
@@ -283,7 +287,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     Sn[g][j] = __ldg(P.fSq + base + tl);
                     if (base + tl < P.n_theta) valid_bits |= 1u << (2 * g + j);
                 }
-            __syncthreads();  // tile zeroed, hits staged, strip list consumed
+            __syncthreads();  // tile zeroed, hits staged
             HOUGH_PT(1);
             {
                 const int ns = sh.n_safe, nu = sh.n_unsafe;
@@ -304,9 +308,12 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                         c = halo[P.n_rho + r];
                         pk = c >= T && fis_peak(P, tile, halo, base, -1, r, c);
                     }
-                    const int i = warp_append(&sh.n_peaks, pk);
+                    const int ip = warp_append(&sh.n_peaks, pk);
                     if (pk) {
-                        if (i < P.fPCAP) peaks[i] = ((kCountMax - c) << kLBits) | (uint32_t)((base - 1) * P.n_rho + r);
+                        if (ip < P.fPCAP) {
+                            peaks[ip] = ((kCountMax - c) << kLBits) | (uint32_t)((base - 1) * P.n_rho + r);
+                            pidx[ip] = (uint16_t)(ihalo_prev[r] & 0x7fffu);
+                        }
                         atomicAdd(&hist[min(c, 255u)], 1);
                     }
                 }
@@ -321,14 +328,10 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     if (idx < total) {
                         w = t4[idx];
                         const uint32_t gx = __vcmpgeu2(w.x, TT), gy = __vcmpgeu2(w.y, TT), gz = __vcmpgeu2(w.z, TT), gw = __vcmpgeu2(w.w, TT);
-                        if (gx | gy | gz | gw) {
+                        if (gx | gy | gz | gw)
                             m = ((gx & 1u) | ((gx >> 15) & 2u)) | (((gy & 1u) | ((gy >> 15) & 2u)) << 2) |
                                 (((gz & 1u) | ((gz >> 15) & 2u)) << 4) | (((gw & 1u) | ((gw >> 15) & 2u)) << 6);
-                            if (!full) {  // theta rows beyond n_theta hold no votes, but keep the mask exact anyway
-                                const int tl0 = (idx & (cpr - 1)) * 8;
-                                for (int q = 0; q < 8; ++q) if (base + tl0 + q >= P.n_theta) m &= ~(1u << q);
-                            }
-                        }
+                        // theta rows beyond n_theta hold no votes (checked_vote masks them), so m needs no masking
                     }
                     if (__ballot_sync(0xffffffffu, m != 0) == 0) continue;
                     const int cnt = __popc(m);
@@ -354,64 +357,96 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             }
             __syncthreads();
             HOUGH_PT(4);
-            // ---------------- one thread per on bin: global on list, local-maximum test
-            {
-                const int n_sl = sh.n_sl;
-                const int on0 = sh.n_on;
-                if (n_sl > P.fSLCAP) sh.defer = 1;  // benign race: every writer stores 1
-                const int n_do = min(n_sl, P.fSLCAP);
-                for (int i0 = tid - lane; i0 < n_do; i0 += nthr) {
-                    const int i = i0 + lane;
-                    bool pk = false;
-                    uint32_t c = 0, L = 0;
-                    if (i < n_do) {
-                        const uint32_t ent = slist[i];
-                        c = ent & kCountMax;
-                        const int loc = (int)(ent >> kCountBits);
-                        const int r = loc >> (k - 1), tl = loc & (S - 1);  // S = 2^(k-1) theta rows per strip
-                        L = (uint32_t)((base + tl) * P.n_rho + r);
-                        if (on0 + i < P.f_oncap) __stcg(onlist + on0 + i, L);
-                        pk = (tl < S - 1 || last_strip) && fis_peak(P, tile, halo, base, tl, r, c);
-                    }
-                    const int ip = warp_append(&sh.n_peaks, pk);
-                    if (pk) {
-                        if (ip < P.fPCAP) peaks[ip] = ((kCountMax - c) << kLBits) | L;
-                        atomicAdd(&hist[min(c, 255u)], 1);
-                    }
+            const int n_sl = sh.n_sl, on0 = sh.n_on;
+            if (sh.defer || n_sl > P.fSLCAP || on0 + n_sl > P.f_oncap) { give_up = true; break; }  // block-uniform
+
+            // ---------------- (a) one thread per on bin: local-maximum test on the counts
+            for (int i0 = tid - lane; i0 < n_sl; i0 += nthr) {
+                const int i = i0 + lane;
+                bool pk = false;
+                uint32_t c = 0, L = 0;
+                if (i < n_sl) {
+                    const uint32_t ent = slist[i];
+                    c = ent & kCountMax;
+                    const int loc = (int)(ent >> kCountBits);
+                    const int r = loc >> (k - 1), tl = loc & (S - 1);  // S = 2^(k-1) theta rows per strip
+                    L = (uint32_t)((base + tl) * P.n_rho + r);
+                    pk = (tl < S - 1 || last_strip) && fis_peak(P, tile, halo, base, tl, r, c);
+                }
+                const int ip = warp_append(&sh.n_peaks, pk);
+                if (pk) {
+                    if (ip < P.fPCAP) { peaks[ip] = ((kCountMax - c) << kLBits) | L; pidx[ip] = (uint16_t)(on0 + i); }
+                    atomicAdd(&hist[min(c, 255u)], 1);
                 }
             }
-            __syncthreads();
-            HOUGH_PT(5);
-            if (tid == 0) { sh.n_on += sh.n_sl; sh.n_sl = 0; }
-            if (!last_strip) {  // keep the last two theta rows for the next strip's tests
+            __syncthreads();  // every count of the strip has been read: the halo and the tile entries may change
+            if (!last_strip) {  // keep the counts of the last two theta rows for the next strip's tests
                 for (int r = tid; r < P.n_rho; r += nthr) {
                     halo[r] = tile[r * S + S - 2];
                     halo[P.n_rho + r] = tile[r * S + S - 1];
                 }
             }
+            __syncthreads();
+            // ---------------- (b) on bins become kOnFlag | on-list index; singleton sets
+            for (int i = tid; i < n_sl; i += nthr) {
+                const int loc = (int)(slist[i] >> kCountBits);
+                tile[loc] = (uint16_t)(kOnFlag | (uint32_t)(on0 + i));
+                parent[on0 + i] = (unsigned short)(on0 + i);
+            }
+            __syncthreads();
+            HOUGH_PT(5);
+            // ---------------- (c) S3: join with the four neighbours that have a smaller linear index
+            for (int i0 = tid - lane; i0 < n_sl; i0 += nthr) {
+                const int i = i0 + lane;
+                if (i < n_sl) {
+                    const int loc = (int)(slist[i] >> kCountBits);
+                    const int r = loc >> (k - 1), tl = loc & (S - 1);
+                    const uint32_t me = (uint32_t)(on0 + i);
+                    const uint32_t n0 = fentry_at(P, tile, ihalo_prev, tl, r - 1);
+                    const uint32_t n1 = fentry_at(P, tile, ihalo_prev, tl - 1, r);
+                    if (n0 & kOnFlag) suf_union(parent, me, n0 & 0x7fffu);
+                    if (n1 & kOnFlag) suf_union(parent, me, n1 & 0x7fffu);
+                    else {  // (t-1, r-1) and (t-1, r+1) are already joined through (t-1, r) when that bin is on
+                        const uint32_t n2 = fentry_at(P, tile, ihalo_prev, tl - 1, r - 1);
+                        const uint32_t n3 = fentry_at(P, tile, ihalo_prev, tl - 1, r + 1);
+                        if (n2 & kOnFlag) suf_union(parent, me, n2 & 0x7fffu);
+                        if (n3 & kOnFlag) suf_union(parent, me, n3 & 0x7fffu);
+                    }
+                }
+                __syncwarp();  // reconverge after the data-dependent union loops
+            }
+            if (!last_strip) {  // entries of the last theta row, for the next strip's joins and deferred-row peaks
+                for (int r = tid; r < P.n_rho; r += nthr) {
+                    const uint16_t en = tile[r * S + S - 1];
+                    ihalo_cur[r] = (en & kOnFlag) ? en : (uint16_t)0;
+                }
+            }
+            if (tid == 0) { sh.n_on = on0 + n_sl; sh.n_sl = 0; }
             __syncthreads();  // the tile may be zeroed again
             HOUGH_PT(6);
         }  // strips
 
         const int n_on = sh.n_on, n_pk = sh.n_peaks;
-        if (sh.defer || n_on > P.f_oncap || n_pk > P.fPCAP) {
+        if (give_up || n_pk > P.fPCAP) {
             if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
             continue;
         }
+        // the tile is dead: its first ONCAP halfwords become the root tags
+        for (int i = tid; i < (n_on + 1) / 2; i += nthr) reinterpret_cast<uint32_t*>(roottag)[i] = 0;
 
-        // ---------------- S4a: the K best peaks (key = (1023 - votes) << 22 | L, ascending)
+        // ---------------- S4: the K best peaks (key = (1023 - votes) << 22 | L, ascending)
         if (n_pk > P.K) {
             if (tid < 32) {  // threshold vote count c*: #(votes > c*) < K <= #(votes >= c*)
-                int loc[8], s = 0;
+                int s = 0;
 #pragma unroll
-                for (int j = 0; j < 8; ++j) { loc[j] = hist[255 - (lane * 8 + j)]; s += loc[j]; }  // descending votes
+                for (int j = 0; j < 8; ++j) s += hist[255 - (lane * 8 + j)];  // descending votes
                 int incl = s;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
                 int before = incl - s;
                 if (before < P.K && P.K <= incl) {
                     int j = 0;
-                    while (before + loc[j] < P.K) { before += loc[j]; ++j; }
+                    while (before + hist[255 - (lane * 8 + j)] < P.K) { before += hist[255 - (lane * 8 + j)]; ++j; }
                     sh.cstar = 255 - (lane * 8 + j);
                     sh.n_gt = before;
                 }
@@ -422,32 +457,35 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
                 continue;
             }
+            const int tcap = P.fSLCAP >> 1;  // tie list: keys in the first half of the strip list, peak positions in the second
+            uint32_t* tie_key = slist;
+            uint32_t* tie_pos = slist + tcap;
             for (int i0 = tid - lane; i0 < n_pk; i0 += nthr) {
                 const int i = i0 + lane;
                 uint32_t key = 0;
                 int c = -1;
                 if (i < n_pk) { key = peaks[i]; c = (int)(kCountMax - (key >> kLBits)); }
                 const int a = warp_append(&sh.n_kept, c > cstar);
-                if (c > cstar) kept[a] = key;
+                if (c > cstar) { kept[a] = key; kidx[a] = pidx[i]; }
                 const int b = warp_append(&sh.n_ties, c == cstar);
-                if (c == cstar && b < P.fSLCAP) slist[b] = key;
+                if (c == cstar && b < tcap) { tie_key[b] = key; tie_pos[b] = (uint32_t)i; }
             }
             __syncthreads();
             const int n_ties = sh.n_ties, n_gt = sh.n_kept;
-            if (n_ties > P.fSLCAP) {
+            if (n_ties > tcap) {
                 if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
                 continue;
             }
             const int need = P.K - n_gt;  // 1 <= need <= n_ties: the `need` smallest keys among the ties
             for (int i = tid; i < n_ties; i += nthr) {
-                const uint32_t key = slist[i];
+                const uint32_t key = tie_key[i];
                 int rank = 0;
-                for (int j = 0; j < n_ties; ++j) rank += (slist[j] < key);
-                if (rank < need) kept[n_gt + rank] = key;
+                for (int j = 0; j < n_ties; ++j) rank += (tie_key[j] < key);
+                if (rank < need) { kept[n_gt + rank] = key; kidx[n_gt + rank] = pidx[tie_pos[i]]; }
             }
             if (tid == 0) sh.n_kept = P.K;
         } else {
-            for (int i = tid; i < n_pk; i += nthr) kept[i] = peaks[i];
+            for (int i = tid; i < n_pk; i += nthr) { kept[i] = peaks[i]; kidx[i] = pidx[i]; }
             if (tid == 0) sh.n_kept = n_pk;
         }
         __syncthreads();
@@ -457,66 +495,27 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             int s = 0;
             for (int j = 0; j < n_kept; ++j) s += (kept[j] < key);
             sorted[s] = key;
+            sidx[s] = kidx[i];
             ksize[i] = 0;
         }
-        __syncthreads();  // peaks, hist, strip list and tile are dead from here on
+        __syncthreads();
         HOUGH_PT(7);
 
-        // ---------------- S3: connected components of the on mask: hash (L -> slot) + union-find over slots
-        {
-            uint4* h4 = reinterpret_cast<uint4*>(hkeys);
-            for (int i = tid; i < NS / 4; i += nthr) h4[i] = make_uint4(kHashEmpty, kHashEmpty, kHashEmpty, kHashEmpty);
-        }
-        __syncthreads();
-        const uint32_t hmsk = (uint32_t)NS - 1u;
-        for (int i = tid; i < n_on; i += nthr) {
-            const uint32_t L = __ldcg(onlist + i);
-            uint32_t s = hash_slot(L, P.fnsbits);
-            while (atomicCAS(hkeys + s, kHashEmpty, L) != kHashEmpty) s = (s + 1) & hmsk;
-            hparent[s] = (unsigned short)s;
-        }
-        __syncthreads();
-        HOUGH_PT(8);
-        // NS and nthr are multiples of 32, so the trip count is warp-uniform; __syncwarp() makes the lanes reconverge after
-        // the data-dependent probe / union loops of each trip (without it the warp stays split and runs lane by lane)
-        for (int s = tid; s < NS; s += nthr) {
-            const uint32_t L = hkeys[s];
-            if (L != kHashEmpty) {
-                int t, r;
-                split_L(P, L, t, r);
-                // the four neighbours with a smaller linear index; each adjacent pair is visited exactly once
-                const uint32_t up = L - (uint32_t)P.n_rho;
-                const int n0 = (r > 0) ? hash_find(hkeys, L - 1, P.fnsbits) : -1;
-                const int n1 = (t > 0) ? hash_find(hkeys, up, P.fnsbits) : -1;
-                const int n2 = (t > 0 && r > 0) ? hash_find(hkeys, up - 1, P.fnsbits) : -1;
-                const int n3 = (t > 0 && r + 1 < P.n_rho) ? hash_find(hkeys, up + 1, P.fnsbits) : -1;
-                if (n0 >= 0) suf_union(hparent, (uint32_t)s, (uint32_t)n0);
-                if (n1 >= 0) suf_union(hparent, (uint32_t)s, (uint32_t)n1);
-                else {  // (t-1, r-1) and (t-1, r+1) are already joined through (t-1, r) when that bin is on
-                    if (n2 >= 0) suf_union(hparent, (uint32_t)s, (uint32_t)n2);
-                    if (n3 >= 0) suf_union(hparent, (uint32_t)s, (uint32_t)n3);
-                }
-            }
-            __syncwarp();
-        }
-        __syncthreads();
-        HOUGH_PT(9);
-        for (int s = tid; s < n_kept; s += nthr)
-            kroot[s] = suf_find(hparent, (uint32_t)hash_find(hkeys, sorted[s] & kLMask, P.fnsbits));
+        // ---------------- cluster of each kept peak: root, best-ranked kept peak of the same cluster, size
+        for (int s = tid; s < n_kept; s += nthr) kroot[s] = suf_find(parent, (uint32_t)sidx[s]);
         __syncthreads();
         for (int s = tid; s < n_kept; s += nthr) {
             const uint32_t root = kroot[s];
             int rs = 0;
             while (kroot[rs] != root) ++rs;  // best-ranked kept peak of the same component (<= s)
-            // tag the root slot with rs + 1 in the 10 spare bits of its key (every peak of the component writes the same value)
-            if (rs == s) hkeys[root] = (hkeys[root] & kLMask) | ((uint32_t)(rs + 1) << kLBits);
+            if (rs == s) roottag[root] = (uint16_t)(s + 1);
         }
         __syncthreads();
-        for (int s = tid; s < NS; s += nthr) {  // sizes of the components that own a kept peak
-            const uint32_t key = hkeys[s];
-            if (key != kHashEmpty) {
-                const uint32_t root = suf_find(hparent, (uint32_t)s);
-                const uint32_t id = hkeys[root] >> kLBits;
+        HOUGH_PT(8);
+        for (int i0 = tid - lane; i0 < n_on; i0 += nthr) {  // sizes of the components that own a kept peak
+            const int i = i0 + lane;
+            if (i < n_on) {
+                const uint32_t id = roottag[suf_find(parent, (uint32_t)i)];
                 if (id != 0) atomicAdd(ksize + (id - 1), 1u);
             }
             __syncwarp();
@@ -524,14 +523,12 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
         __syncthreads();
         HOUGH_PT(10);
 
-        // ---------------- S4b: records in rank order
+        // ---------------- records in rank order
         for (int s = tid; s < n_kept; s += nthr) {
             const uint32_t key = sorted[s];
             const uint32_t L = key & kLMask;
             const uint32_t c = kCountMax - (key >> kLBits);
-            const uint32_t root = kroot[s];
-            int rs = 0;
-            while (kroot[rs] != root) ++rs;
+            const int rs = (int)roottag[kroot[s]] - 1;
             int t, r;
             split_L(P, L, t, r);
             const float th = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)t), (double)P.n_theta);

@@ -59,12 +59,11 @@ struct DevParams {
     int rho_shift;                   // log2(n_rho) if n_rho is a power of two, else -1
     int fk, fsh;                     // log2(row bytes), F - fk
     int fS, f_nstrips, f_tile_bytes; // theta rows per strip (64 G), strips per event
-    int fHB, fSLCAP, fPCAP, fnsbits; // staged hits, strip list, peak list, log2(hash slots)
-    int f_oncap;                     // on bins an event may have on the fast path (3/4 of the hash slots)
-    int f_off_hits, f_off_halo, f_off_slist, f_off_peaks, f_off_hist, f_off_kept;
+    int fHB, fSLCAP, fPCAP;          // capacities: staged hits, strip list, peak list
+    int f_oncap;                     // on bins an event may have on the fast path (union-find parents)
+    int f_off_hits, f_off_halo, f_off_ihalo, f_off_slist, f_off_peaks, f_off_pidx, f_off_parent, f_off_hist, f_off_kept;
     const int* fCq;                  // [f_nstrips * fS], zero padded
     const int* fSq;
-    uint32_t* f_onlist;              // [n_fast_ctas][f_oncap] linear indices of the on bins of the current event
     int* deferred;                   // [max_events] events the fast kernel left to the general kernel
     unsigned int* deferred_count;
     unsigned int* f_work_counter;

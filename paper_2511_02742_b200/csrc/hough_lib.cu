@@ -46,7 +46,6 @@ struct hough_plan {
     int f_G, f_maxt, f_minb, f_threads, f_ctas, f_smem;
     int* d_fcos;
     int* d_fsin;
-    uint32_t* d_fonlist;
     int* d_deferred;
     // owned device memory
     int* d_cos;
@@ -163,18 +162,21 @@ static cudaError_t dispatch_fast(const hough_plan* p, const float* u, const floa
 }
 
 struct FastLayout {
-    int off_hits, off_halo, off_slist, off_peaks, off_hist, off_kept, total;
+    int off_hits, off_halo, off_ihalo, off_slist, off_peaks, off_pidx, off_parent, off_hist, off_kept, total;
 };
-static FastLayout layout_fast(int tile_bytes, int HB, int n_rho, int SLCAP, int PCAP, int K)
+static FastLayout layout_fast(int tile_bytes, int HB, int n_rho, int SLCAP, int PCAP, int ONCAP, int K)
 {
     FastLayout L;
     size_t o = align_up((size_t)tile_bytes, 16);
     L.off_hits = (int)o;   o = align_up(o + (size_t)HB * 8, 16);
     L.off_halo = (int)o;   o = align_up(o + (size_t)2 * n_rho * 2, 16);
+    L.off_ihalo = (int)o;  o = align_up(o + (size_t)2 * n_rho * 2, 16);
     L.off_slist = (int)o;  o = align_up(o + (size_t)SLCAP * 4, 16);
     L.off_peaks = (int)o;  o = align_up(o + (size_t)PCAP * 4, 16);
+    L.off_pidx = (int)o;   o = align_up(o + (size_t)PCAP * 2, 16);
+    L.off_parent = (int)o; o = align_up(o + (size_t)ONCAP * 2, 16);
     L.off_hist = (int)o;   o = align_up(o + 256 * 4, 16);
-    L.off_kept = (int)o;   o = align_up(o + (size_t)K * 16, 16);
+    L.off_kept = (int)o;   o = align_up(o + (size_t)K * 20, 16);
     o += 64;               // FastShared control block
     L.total = (int)o;
     return L;
@@ -315,14 +317,14 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     p->assign_ctas = n_sm * 8;
     p->launches = 0;
 
-    // ---- fast kernel configuration (hough_fast.cuh): u16 counters, rows of 128 G bytes, several CTAs per SM
+    // ---- fast kernel configuration (hough_fast.cuh): u16 counters, tile rows of 128 G bytes
     p->f_G = 0;
     FastLayout flay{};
-    int f_S = 0, f_nstrips = 0, f_tile = 0, f_HB = 0, f_SLCAP = 0, f_PCAP = 0, f_nsbits = 0, f_k = 0;
+    int f_S = 0, f_nstrips = 0, f_tile = 0, f_HB = 0, f_SLCAP = 0, f_PCAP = 0, f_ONCAP = 0, f_k = 0;
     if (cw == 2 && d->vote_threshold <= 1023 && K <= 1000 && d->max_hits_per_event >= 1 && !env_int("HOUGH_NO_FAST", 0)) {
         struct Cand { int G, maxt, minb, threads, cps; };
-        // preference order: two co-resident CTAs (overlap of vote and scan/cluster phases), widest rows first
-        const Cand cands[] = {{4, 768, 2, 768, 2}, {2, 768, 2, 768, 2}, {1, 768, 2, 768, 2}, {4, 1024, 1, 1024, 1}, {2, 1024, 1, 1024, 1}, {1, 1024, 1, 1024, 1}};
+        // preference order: one 1024-thread CTA per SM with the widest tile row that fits, then two CTAs per SM
+        const Cand cands[] = {{4, 1024, 1, 1024, 1}, {2, 1024, 1, 1024, 1}, {1, 1024, 1, 1024, 1}, {4, 768, 2, 768, 2}, {2, 768, 2, 768, 2}, {1, 768, 2, 768, 2}};
         const int want_G = env_int("HOUGH_FAST_G", 0), want_t = env_int("HOUGH_FAST_MAXT", 0), want_b = env_int("HOUGH_FAST_MINB", 0);
         const int want_threads = env_int("HOUGH_FAST_THREADS", 0);
         std::vector<Cand> list(cands, cands + sizeof(cands) / sizeof(cands[0]));
@@ -333,25 +335,28 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
             int kk = 7; while ((128 << (kk - 7)) < 128 * c.G) ++kk;
             const int sh = F - kk;
             if (sh < 0) continue;
-            // unsigned range of a' = a + (tile_base << sh): tile_base < 4096 (static shared memory + alignment)
+            // unsigned range of a' = a + (tile_base << sh): tile_base < 4096 (window offset of the dynamic allocation)
             if (((unsigned long long)4096 << sh) + ((unsigned long long)d->n_rho << F) > 0xffffffffull) continue;
             const int budget = (c.cps == 1 ? smem_optin : (smem_sm / c.cps - reserved)) - 128;  // the kernel has no static shared memory
             const int lim = budget < smem_optin ? budget : smem_optin;
             const int tile = d->n_rho * 128 * c.G;
+            if ((long long)d->n_rho * rows >= (1ll << 17)) continue;  // strip-list entries hold a 17-bit tile index
             int hb = (int)align_up((size_t)(d->max_hits_per_event < 32 ? 32 : d->max_hits_per_event), 32);
             if (hb > 8192) hb = 8192;
-            int slcap = env_int("HOUGH_FAST_SLCAP", 2048), pcap = env_int("HOUGH_FAST_PCAP", 4096);
-            while (layout_fast(tile, hb, d->n_rho, slcap, pcap, K).total > lim && pcap > 2048) pcap -= 256;
-            while (layout_fast(tile, hb, d->n_rho, slcap, pcap, K).total > lim && slcap > 1024) slcap -= 256;
-            while (layout_fast(tile, hb, d->n_rho, slcap, pcap, K).total > lim && hb > 1024) hb -= 32;
-            const FastLayout L = layout_fast(tile, hb, d->n_rho, slcap, pcap, K);
+            int slcap = env_int("HOUGH_FAST_SLCAP", 2048 * c.G > 8192 ? 8192 : 2048 * c.G), pcap = env_int("HOUGH_FAST_PCAP", 4096);
+            int oncap = env_int("HOUGH_FAST_ONCAP", 12288);
+            if (oncap > 32767) oncap = 32767;
+            if (oncap * 2 > tile) oncap = tile / 2;  // root tags reuse the tile
+            auto total = [&]() { return layout_fast(tile, hb, d->n_rho, slcap, pcap, oncap, K).total; };
+            while (total() > lim && pcap > 2048) pcap -= 256;
+            while (total() > lim && oncap > 6144) oncap -= 512;
+            while (total() > lim && slcap > 1024) slcap -= 256;
+            while (total() > lim && hb > 1024) hb -= 32;
+            const FastLayout L = layout_fast(tile, hb, d->n_rho, slcap, pcap, oncap, K);
             if (L.total > lim) continue;
-            int nsb = 16;
-            while (nsb > 8 && (size_t)6 << nsb > (size_t)L.off_kept) --nsb;
-            if ((size_t)6 << nsb > (size_t)L.off_kept) continue;
             p->f_G = c.G; p->f_maxt = c.maxt; p->f_minb = c.minb; p->f_threads = c.threads; p->f_ctas = n_sm * c.cps; p->f_smem = L.total;
             flay = L; f_S = rows; f_nstrips = (d->n_theta + rows - 1) / rows; f_tile = tile; f_HB = hb; f_SLCAP = slcap; f_PCAP = pcap;
-            f_nsbits = nsb; f_k = kk;
+            f_ONCAP = oncap; f_k = kk;
             break;
         }
     }
@@ -373,7 +378,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     ok = ok && (ce = cudaMemcpy(p->d_sin, pads.data(), tab * 4, cudaMemcpyHostToDevice)) == cudaSuccess;
     ok = ok && (ce = cudaMemset(p->d_scratch, 0, scratch_bytes)) == cudaSuccess;
     ok = ok && (ce = cudaMemset(p->d_status, 0, 256)) == cudaSuccess;
-    const int f_oncap = p->f_G ? (3 << f_nsbits) / 4 : 0;
+    const int f_oncap = f_ONCAP;
     if (p->f_G) {
         const size_t ftab = (size_t)f_nstrips * f_S;
         std::vector<int32_t> fc(ftab, 0), fs(ftab, 0);
@@ -381,7 +386,6 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
         memcpy(fs.data(), p->h_sin.data(), sizeof(int32_t) * d->n_theta);
         ok = ok && (ce = cudaMalloc((void**)&p->d_fcos, ftab * 4)) == cudaSuccess;
         ok = ok && (ce = cudaMalloc((void**)&p->d_fsin, ftab * 4)) == cudaSuccess;
-        ok = ok && (ce = cudaMalloc((void**)&p->d_fonlist, (size_t)p->f_ctas * f_oncap * 4)) == cudaSuccess;
         ok = ok && (ce = cudaMalloc((void**)&p->d_deferred, (size_t)d->max_events * 4)) == cudaSuccess;
         ok = ok && (ce = cudaMemcpy(p->d_fcos, fc.data(), ftab * 4, cudaMemcpyHostToDevice)) == cudaSuccess;
         ok = ok && (ce = cudaMemcpy(p->d_fsin, fs.data(), ftab * 4, cudaMemcpyHostToDevice)) == cudaSuccess;
@@ -440,10 +444,11 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     for (int b = 0; b < 31; ++b) if ((1 << b) == d->n_rho) P.rho_shift = b;
     if (p->f_G) {
         P.fk = f_k; P.fsh = F - f_k; P.fS = f_S; P.f_nstrips = f_nstrips; P.f_tile_bytes = f_tile;
-        P.fHB = f_HB; P.fSLCAP = f_SLCAP; P.fPCAP = f_PCAP; P.fnsbits = f_nsbits; P.f_oncap = f_oncap;
-        P.f_off_hits = flay.off_hits; P.f_off_halo = flay.off_halo; P.f_off_slist = flay.off_slist;
-        P.f_off_peaks = flay.off_peaks; P.f_off_hist = flay.off_hist; P.f_off_kept = flay.off_kept;
-        P.fCq = p->d_fcos; P.fSq = p->d_fsin; P.f_onlist = p->d_fonlist; P.deferred = p->d_deferred;
+        P.fHB = f_HB; P.fSLCAP = f_SLCAP; P.fPCAP = f_PCAP; P.f_oncap = f_oncap;
+        P.f_off_hits = flay.off_hits; P.f_off_halo = flay.off_halo; P.f_off_ihalo = flay.off_ihalo; P.f_off_slist = flay.off_slist;
+        P.f_off_peaks = flay.off_peaks; P.f_off_pidx = flay.off_pidx; P.f_off_parent = flay.off_parent;
+        P.f_off_hist = flay.off_hist; P.f_off_kept = flay.off_kept;
+        P.fCq = p->d_fcos; P.fSq = p->d_fsin; P.deferred = p->d_deferred;
     }
     P.phase_cycles = reinterpret_cast<unsigned long long*>(p->d_status) + 16;  // bytes 128..255 of the status block
 
@@ -465,7 +470,7 @@ int hough_plan_destroy(hough_plan_t* p)
     (void)cudaSetDevice(p->desc.device);
     (void)cudaDeviceSynchronize();
     cudaFree(p->d_cos); cudaFree(p->d_sin); cudaFree(p->d_scratch); cudaFree(p->d_status);
-    cudaFree(p->d_fcos); cudaFree(p->d_fsin); cudaFree(p->d_fonlist); cudaFree(p->d_deferred);
+    cudaFree(p->d_fcos); cudaFree(p->d_fsin); cudaFree(p->d_deferred);
     cudaFree(p->hd_u); cudaFree(p->hd_v); cudaFree(p->hd_off); cudaFree(p->hd_cands); cudaFree(p->hd_nfound); cudaFree(p->hd_labels);
     if (p->h_stream) cudaStreamDestroy(p->h_stream);
     (void)cudaGetLastError();
