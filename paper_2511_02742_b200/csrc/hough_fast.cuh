@@ -158,29 +158,6 @@ __device__ __forceinline__ void checked_vote(const DevParams& P, const int2* __r
     }
 }
 
-// Count at (strip-local theta row tl, rho bin r) for the strip whose first theta row is `base`; rows -2 and -1 come from
-// the halo saved from the previous strip; anything outside the grid counts as 0.
-__device__ __forceinline__ uint32_t fcount_at(const DevParams& P, const uint16_t* tile, const uint16_t* halo, int base, int tl, int r)
-{
-    if ((unsigned)r >= (unsigned)P.n_rho) return 0;
-    if (tl >= 0) return (tl < P.fS && base + tl < P.n_theta) ? tile[r * P.fS + tl] : 0;
-    return halo[(tl + 2) * P.n_rho + r];
-}
-
-__device__ __forceinline__ bool fis_peak(const DevParams& P, const uint16_t* tile, const uint16_t* halo, int base, int tl, int r, uint32_t c)
-{
-    if (fcount_at(P, tile, halo, base, tl - 1, r - 1) >= c) return false;
-    if (fcount_at(P, tile, halo, base, tl - 1, r) >= c) return false;
-    if (fcount_at(P, tile, halo, base, tl - 1, r + 1) >= c) return false;
-    if (fcount_at(P, tile, halo, base, tl, r - 1) >= c) return false;
-    if (fcount_at(P, tile, halo, base, tl, r + 1) > c) return false;
-    if (fcount_at(P, tile, halo, base, tl + 1, r - 1) > c) return false;
-    if (fcount_at(P, tile, halo, base, tl + 1, r) > c) return false;
-    if (fcount_at(P, tile, halo, base, tl + 1, r + 1) > c) return false;
-    return true;
-}
-
-
 // Tile entry of bin (strip-local theta row tl, rho bin r) after step (b): kOnFlag | on-list index for an on bin, a
 // count below the threshold otherwise.  Row -1 is the previous strip's last row (index halo); outside the grid -> 0.
 __device__ __forceinline__ uint32_t fentry_at(const DevParams& P, const uint16_t* tile, const uint16_t* ihalo_prev, int tl, int r)
@@ -202,7 +179,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 
     uint16_t* tile = reinterpret_cast<uint16_t*>(smem);
     int2* hits = reinterpret_cast<int2*>(smem + P.f_off_hits);
-    uint16_t* halo = reinterpret_cast<uint16_t*>(smem + P.f_off_halo);      // [2][n_rho] counts of the previous strip's last two rows
+    uint16_t* halo = reinterpret_cast<uint16_t*>(smem + P.f_off_halo);      // [2][2][n_rho] counts of a strip's last two rows, by strip parity
     uint16_t* ihalo = reinterpret_cast<uint16_t*>(smem + P.f_off_ihalo);    // [2][n_rho] entries of a strip's last row, by strip parity
     uint32_t* slist = reinterpret_cast<uint32_t*>(smem + P.f_off_slist);    // strip list; later the tie list
     uint32_t* peaks = reinterpret_cast<uint32_t*>(smem + P.f_off_peaks);    // [PCAP] packed keys
@@ -215,7 +192,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
     uint32_t* ksize = kroot + P.K;
     uint16_t* kidx = reinterpret_cast<uint16_t*>(ksize + P.K);              // [K] on-list index, unordered / sorted
     uint16_t* sidx = kidx + P.K;
-    uint16_t* roottag = tile;  // after the last strip: [ONCAP] slot + 1 of the component's best kept peak, at union-find roots
+    uint32_t* roottag = reinterpret_cast<uint32_t*>(tile);  // after the last strip: [ONCAP] K - slot of the best kept peak, at roots
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
     const uint32_t tile_base = smem_addr(tile);
@@ -227,7 +204,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
     for (int g = 0; g < G; ++g) col[g] = 4u * lane + 128u * g;
     const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe, P.fHB};
     const uint32_t T = (uint32_t)P.T;
-    const uint32_t TT = T | (T << 16);
+    const uint32_t tadd = (0x8000u - T) * 0x00010001u;
     const int cpr = 8 * G;  // 16-byte chunks per rho row
 #ifdef HOUGH_PHASE_TIMERS
     long long pt_acc[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -256,10 +233,12 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             if (tid == 0) n_found[e] = 0;
             continue;
         }
-        for (int i = tid; i < P.n_rho; i += nthr) {  // both count-halo rows and both index-halo rows (u16 pairs)
+        for (int i = tid; i < P.n_rho; i += nthr) {  // count halos (2 x 2 rows) and index halos (2 rows), as u16 pairs
             reinterpret_cast<uint32_t*>(halo)[i] = 0;
+            reinterpret_cast<uint32_t*>(halo)[P.n_rho + i] = 0;
             reinterpret_cast<uint32_t*>(ihalo)[i] = 0;
         }
+        const int r_lo = 0, r_hi = P.n_rho - 1;
         for (int i = tid; i < 256; i += nthr) hist[i] = 0;
         stage_hits(P, sc, u, v, g0, ne);
         HOUGH_PT(0);
@@ -271,6 +250,8 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             const bool full = base + S <= P.n_theta;
             const uint16_t* ihalo_prev = ihalo + ((strip + 1) & 1) * P.n_rho;  // written by the previous strip
             uint16_t* ihalo_cur = ihalo + (strip & 1) * P.n_rho;
+            const uint16_t* halo_prev = halo + ((strip + 1) & 1) * 2 * P.n_rho;
+            uint16_t* halo_cur = halo + (strip & 1) * 2 * P.n_rho;
             {
                 uint4* t4 = reinterpret_cast<uint4*>(tile);
                 const int n16 = P.f_tile_bytes >> 4;
@@ -299,38 +280,22 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             HOUGH_PT(3);
 
             // ---------------- S2: threshold, compaction of the strip's on bins
-            if (strip > 0) {  // deferred row: the last theta row of the previous strip, now that row 0 is known
-                for (int r0 = tid - lane; r0 < P.n_rho; r0 += nthr) {
-                    const int r = r0 + lane;
-                    uint32_t c = 0;
-                    bool pk = false;
-                    if (r < P.n_rho) {
-                        c = halo[P.n_rho + r];
-                        pk = c >= T && fis_peak(P, tile, halo, base, -1, r, c);
-                    }
-                    const int ip = warp_append(&sh.n_peaks, pk);
-                    if (pk) {
-                        if (ip < P.fPCAP) {
-                            peaks[ip] = ((kCountMax - c) << kLBits) | (uint32_t)((base - 1) * P.n_rho + r);
-                            pidx[ip] = (uint16_t)(ihalo_prev[r] & 0x7fffu);
-                        }
-                        atomicAdd(&hist[min(c, 255u)], 1);
-                    }
-                }
-            }
             {
-                const int total = P.n_rho * cpr;
                 const uint4* t4 = reinterpret_cast<const uint4*>(tile);
-                for (int i0 = tid - lane; i0 < total; i0 += nthr) {
+                const int i_lo = r_lo * cpr, i_hi = (r_hi + 1) * cpr;  // only rho rows some hit can reach
+                for (int i0 = i_lo + tid - lane; i0 < i_hi; i0 += nthr) {
                     const int idx = i0 + lane;
                     uint32_t m = 0;  // bit q set <=> count q of this chunk is on
                     uint4 w = make_uint4(0, 0, 0, 0);
-                    if (idx < total) {
+                    if (idx < i_hi) {
                         w = t4[idx];
-                        const uint32_t gx = __vcmpgeu2(w.x, TT), gy = __vcmpgeu2(w.y, TT), gz = __vcmpgeu2(w.z, TT), gw = __vcmpgeu2(w.w, TT);
+                        // counts are below 2^15 (at most one vote per hit, fHB <= 32767), so adding 2^15 - T to both
+                        // halfwords sets their top bits exactly where count >= T, without a carry between them
+                        const uint32_t gx = (w.x + tadd) & 0x80008000u, gy = (w.y + tadd) & 0x80008000u;
+                        const uint32_t gz = (w.z + tadd) & 0x80008000u, gw = (w.w + tadd) & 0x80008000u;
                         if (gx | gy | gz | gw)
-                            m = ((gx & 1u) | ((gx >> 15) & 2u)) | (((gy & 1u) | ((gy >> 15) & 2u)) << 2) |
-                                (((gz & 1u) | ((gz >> 15) & 2u)) << 4) | (((gw & 1u) | ((gw >> 15) & 2u)) << 6);
+                            m = (((gx >> 15) | (gx >> 30)) & 3u) | ((((gy >> 15) | (gy >> 30)) & 3u) << 2) |
+                                ((((gz >> 15) | (gz >> 30)) & 3u) << 4) | ((((gw >> 15) | (gw >> 30)) & 3u) << 6);
                         // theta rows beyond n_theta hold no votes (checked_vote masks them), so m needs no masking
                     }
                     if (__ballot_sync(0xffffffffu, m != 0) == 0) continue;
@@ -343,16 +308,25 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     wbase = __shfl_sync(0xffffffffu, wbase, 31);
                     int slot = wbase + incl - cnt;
                     const int r = idx >> (k - 4), tl0 = (idx & (cpr - 1)) * 8;  // cpr = 2^(k-4) chunks per row
+                    const uint32_t heads = m & ~(m << 1);  // first bin of every run of consecutive theta rows in this chunk
                     while (m) {
                         const int q = __ffs(m) - 1;
                         m &= m - 1;
                         const uint32_t wq = (q < 4) ? ((q < 2) ? w.x : w.y) : ((q < 6) ? w.z : w.w);
                         const uint32_t c = (wq >> (16 * (q & 1))) & 0xffffu;
                         if (c > kCountMax) sh.defer = 1;
-                        // strip-list entry: bin index inside the tile (17 bits) | votes (10 bits)
-                        if (slot < P.fSLCAP) slist[slot] = ((uint32_t)(r * S + tl0 + q) << kCountBits) | (c & kCountMax);
+                        const int hoff = q - (31 - __clz(heads & ((2u << q) - 1u)));  // distance to the head of its run (0..7)
+                        // strip-list entry: run-head distance (3 bits) | bin index inside the tile (17 bits) | votes (10 bits)
+                        if (slot < P.fSLCAP)
+                            slist[slot] = ((uint32_t)hoff << 27) | ((uint32_t)(r * S + tl0 + q) << kCountBits) | (c & kCountMax);
                         ++slot;
                     }
+                }
+            }
+            if (!last_strip) {  // counts of the last two theta rows, for the next strip's local-maximum tests
+                for (int r = tid; r < P.n_rho; r += nthr) {
+                    halo_cur[r] = tile[r * S + S - 2];
+                    halo_cur[P.n_rho + r] = tile[r * S + S - 1];
                 }
             }
             __syncthreads();
@@ -360,7 +334,23 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             const int n_sl = sh.n_sl, on0 = sh.n_on;
             if (sh.defer || n_sl > P.fSLCAP || on0 + n_sl > P.f_oncap) { give_up = true; break; }  // block-uniform
 
-            // ---------------- (a) one thread per on bin: local-maximum test on the counts
+            // ---------------- (b) on bins become kOnFlag | on-list index; a bin below another on bin of its chunk joins that
+            //                      run's head right away (indices of one chunk are consecutive), the others are singletons
+            for (int i = tid; i < n_sl; i += nthr) {
+                const uint32_t ent = slist[i];
+                tile[(ent >> kCountBits) & 0x1ffffu] = (uint16_t)(kOnFlag | (uint32_t)(on0 + i));
+                parent[on0 + i] = (unsigned short)(on0 + i - (int)(ent >> 27));
+            }
+            __syncthreads();
+            HOUGH_PT(5);
+
+            // ---------------- (a)+(c) one thread per on bin: local-maximum test and S3 joins, from the same 8 neighbour entries.
+            // A neighbour can beat an on bin only if it is on itself, and then its count is in the strip list (this strip) or in
+            // the count halo (previous strip's last row).
+            auto ncount = [&](uint32_t en, int tl_nb, int r_nb) -> uint32_t {
+                if (!(en & kOnFlag)) return 0u;
+                return tl_nb >= 0 ? (slist[(int)(en & 0x7fffu) - on0] & kCountMax) : (uint32_t)halo_prev[P.n_rho + r_nb];
+            };
             for (int i0 = tid - lane; i0 < n_sl; i0 += nthr) {
                 const int i = i0 + lane;
                 bool pk = false;
@@ -368,52 +358,68 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 if (i < n_sl) {
                     const uint32_t ent = slist[i];
                     c = ent & kCountMax;
-                    const int loc = (int)(ent >> kCountBits);
+                    const int loc = (int)((ent >> kCountBits) & 0x1ffffu), hoff = (int)(ent >> 27);
                     const int r = loc >> (k - 1), tl = loc & (S - 1);  // S = 2^(k-1) theta rows per strip
+                    const uint32_t me = (uint32_t)(on0 + i);
                     L = (uint32_t)((base + tl) * P.n_rho + r);
-                    pk = (tl < S - 1 || last_strip) && fis_peak(P, tile, halo, base, tl, r, c);
+                    const uint32_t n0 = fentry_at(P, tile, ihalo_prev, tl, r - 1);
+                    const uint32_t n1 = fentry_at(P, tile, ihalo_prev, tl - 1, r);
+                    const uint32_t n2 = fentry_at(P, tile, ihalo_prev, tl - 1, r - 1);
+                    const uint32_t n3 = fentry_at(P, tile, ihalo_prev, tl - 1, r + 1);
+                    // joins with the neighbours of smaller linear index; a join is skipped when other joins already imply it
+                    if (hoff > 0 || (n1 & kOnFlag)) {
+                        if (hoff == 0) suf_union(parent, me, n1 & 0x7fffu);
+                        if ((n0 & kOnFlag) && !(n2 & kOnFlag)) suf_union(parent, me, n0 & 0x7fffu);
+                    } else {
+                        if (n0 & kOnFlag) suf_union(parent, me, n0 & 0x7fffu);
+                        else if (n2 & kOnFlag) suf_union(parent, me, n2 & 0x7fffu);
+                        if (n3 & kOnFlag) suf_union(parent, me, n3 & 0x7fffu);
+                    }
+                    if (tl < S - 1 || last_strip) {
+                        pk = ncount(n2, tl - 1, r - 1) < c && ncount(n1, tl - 1, r) < c && ncount(n3, tl - 1, r + 1) < c && ncount(n0, tl, r - 1) < c;
+                        if (pk) {
+                            const bool below = tl + 1 < S && base + tl + 1 < P.n_theta;  // else: beyond the grid (last strip)
+                            const uint32_t n4 = fentry_at(P, tile, ihalo_prev, tl, r + 1);
+                            const uint32_t n5 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r - 1) : 0u;
+                            const uint32_t n6 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r) : 0u;
+                            const uint32_t n7 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r + 1) : 0u;
+                            pk = ncount(n4, tl, r + 1) <= c && ncount(n5, tl + 1, r - 1) <= c && ncount(n6, tl + 1, r) <= c &&
+                                 ncount(n7, tl + 1, r + 1) <= c;
+                        }
+                    }
                 }
+                __syncwarp();  // reconverge after the data-dependent union loops
                 const int ip = warp_append(&sh.n_peaks, pk);
                 if (pk) {
                     if (ip < P.fPCAP) { peaks[ip] = ((kCountMax - c) << kLBits) | L; pidx[ip] = (uint16_t)(on0 + i); }
                     atomicAdd(&hist[min(c, 255u)], 1);
                 }
             }
-            __syncthreads();  // every count of the strip has been read: the halo and the tile entries may change
-            if (!last_strip) {  // keep the counts of the last two theta rows for the next strip's tests
-                for (int r = tid; r < P.n_rho; r += nthr) {
-                    halo[r] = tile[r * S + S - 2];
-                    halo[P.n_rho + r] = tile[r * S + S - 1];
-                }
-            }
-            __syncthreads();
-            // ---------------- (b) on bins become kOnFlag | on-list index; singleton sets
-            for (int i = tid; i < n_sl; i += nthr) {
-                const int loc = (int)(slist[i] >> kCountBits);
-                tile[loc] = (uint16_t)(kOnFlag | (uint32_t)(on0 + i));
-                parent[on0 + i] = (unsigned short)(on0 + i);
-            }
-            __syncthreads();
-            HOUGH_PT(5);
-            // ---------------- (c) S3: join with the four neighbours that have a smaller linear index
-            for (int i0 = tid - lane; i0 < n_sl; i0 += nthr) {
-                const int i = i0 + lane;
-                if (i < n_sl) {
-                    const int loc = (int)(slist[i] >> kCountBits);
-                    const int r = loc >> (k - 1), tl = loc & (S - 1);
-                    const uint32_t me = (uint32_t)(on0 + i);
-                    const uint32_t n0 = fentry_at(P, tile, ihalo_prev, tl, r - 1);
-                    const uint32_t n1 = fentry_at(P, tile, ihalo_prev, tl - 1, r);
-                    if (n0 & kOnFlag) suf_union(parent, me, n0 & 0x7fffu);
-                    if (n1 & kOnFlag) suf_union(parent, me, n1 & 0x7fffu);
-                    else {  // (t-1, r-1) and (t-1, r+1) are already joined through (t-1, r) when that bin is on
-                        const uint32_t n2 = fentry_at(P, tile, ihalo_prev, tl - 1, r - 1);
-                        const uint32_t n3 = fentry_at(P, tile, ihalo_prev, tl - 1, r + 1);
-                        if (n2 & kOnFlag) suf_union(parent, me, n2 & 0x7fffu);
-                        if (n3 & kOnFlag) suf_union(parent, me, n3 & 0x7fffu);
+            if (strip > 0) {  // deferred row: the last theta row of the previous strip, now that row 0 of this one is known
+                for (int r0 = tid - lane; r0 < P.n_rho; r0 += nthr) {
+                    const int r = r0 + lane;
+                    uint32_t c = 0;
+                    bool pk = false;
+                    if (r < P.n_rho) {
+                        c = halo_prev[P.n_rho + r];
+                        if (c >= T) {
+                            const uint32_t lft = r > 0 ? halo_prev[P.n_rho + r - 1] : 0u, rgt = r + 1 < P.n_rho ? halo_prev[P.n_rho + r + 1] : 0u;
+                            const uint32_t a0 = r > 0 ? halo_prev[r - 1] : 0u, a1 = halo_prev[r], a2 = r + 1 < P.n_rho ? halo_prev[r + 1] : 0u;
+                            pk = a0 < c && a1 < c && a2 < c && lft < c && rgt <= c &&
+                                 ncount(fentry_at(P, tile, ihalo_prev, 0, r - 1), 0, r - 1) <= c &&
+                                 ncount(fentry_at(P, tile, ihalo_prev, 0, r), 0, r) <= c &&
+                                 ncount(fentry_at(P, tile, ihalo_prev, 0, r + 1), 0, r + 1) <= c;
+                        }
+                    }
+                    const int ip = warp_append(&sh.n_peaks, pk);
+                    if (pk) {
+                        if (ip < P.fPCAP) {
+                            peaks[ip] = ((kCountMax - c) << kLBits) | (uint32_t)((base - 1) * P.n_rho + r);
+                            pidx[ip] = (uint16_t)(ihalo_prev[r] & 0x7fffu);
+                        }
+                        atomicAdd(&hist[min(c, 255u)], 1);
                     }
                 }
-                __syncwarp();  // reconverge after the data-dependent union loops
             }
             if (!last_strip) {  // entries of the last theta row, for the next strip's joins and deferred-row peaks
                 for (int r = tid; r < P.n_rho; r += nthr) {
@@ -431,8 +437,8 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
             continue;
         }
-        // the tile is dead: its first ONCAP halfwords become the root tags
-        for (int i = tid; i < (n_on + 1) / 2; i += nthr) reinterpret_cast<uint32_t*>(roottag)[i] = 0;
+        // the tile is dead: its first ONCAP words become the root tags
+        for (int i = tid; i < n_on; i += nthr) roottag[i] = 0;
 
         // ---------------- S4: the K best peaks (key = (1023 - votes) << 22 | L, ascending)
         if (n_pk > P.K) {
@@ -502,13 +508,10 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
         HOUGH_PT(7);
 
         // ---------------- cluster of each kept peak: root, best-ranked kept peak of the same cluster, size
-        for (int s = tid; s < n_kept; s += nthr) kroot[s] = suf_find(parent, (uint32_t)sidx[s]);
-        __syncthreads();
         for (int s = tid; s < n_kept; s += nthr) {
-            const uint32_t root = kroot[s];
-            int rs = 0;
-            while (kroot[rs] != root) ++rs;  // best-ranked kept peak of the same component (<= s)
-            if (rs == s) roottag[root] = (uint16_t)(s + 1);
+            const uint32_t root = suf_find(parent, (uint32_t)sidx[s]);
+            kroot[s] = root;
+            atomicMax(roottag + root, (uint32_t)(P.K - s));  // the best-ranked (smallest slot) kept peak of the component wins
         }
         __syncthreads();
         HOUGH_PT(8);
@@ -516,7 +519,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             const int i = i0 + lane;
             if (i < n_on) {
                 const uint32_t id = roottag[suf_find(parent, (uint32_t)i)];
-                if (id != 0) atomicAdd(ksize + (id - 1), 1u);
+                if (id != 0) atomicAdd(ksize + (P.K - id), 1u);
             }
             __syncwarp();
         }
@@ -528,7 +531,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             const uint32_t key = sorted[s];
             const uint32_t L = key & kLMask;
             const uint32_t c = kCountMax - (key >> kLBits);
-            const int rs = (int)roottag[kroot[s]] - 1;
+            const int rs = P.K - (int)roottag[kroot[s]];
             int t, r;
             split_L(P, L, t, r);
             const float th = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)t), (double)P.n_theta);

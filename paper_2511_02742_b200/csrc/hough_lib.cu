@@ -169,7 +169,7 @@ static FastLayout layout_fast(int tile_bytes, int HB, int n_rho, int SLCAP, int 
     FastLayout L;
     size_t o = align_up((size_t)tile_bytes, 16);
     L.off_hits = (int)o;   o = align_up(o + (size_t)HB * 8, 16);
-    L.off_halo = (int)o;   o = align_up(o + (size_t)2 * n_rho * 2, 16);
+    L.off_halo = (int)o;   o = align_up(o + (size_t)4 * n_rho * 2, 16);
     L.off_ihalo = (int)o;  o = align_up(o + (size_t)2 * n_rho * 2, 16);
     L.off_slist = (int)o;  o = align_up(o + (size_t)SLCAP * 4, 16);
     L.off_peaks = (int)o;  o = align_up(o + (size_t)PCAP * 4, 16);
@@ -346,7 +346,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
             int slcap = env_int("HOUGH_FAST_SLCAP", 2048 * c.G > 8192 ? 8192 : 2048 * c.G), pcap = env_int("HOUGH_FAST_PCAP", 4096);
             int oncap = env_int("HOUGH_FAST_ONCAP", 12288);
             if (oncap > 32767) oncap = 32767;
-            if (oncap * 2 > tile) oncap = tile / 2;  // root tags reuse the tile
+            if (oncap * 4 > tile) oncap = tile / 4;  // root tags reuse the tile
             auto total = [&]() { return layout_fast(tile, hb, d->n_rho, slcap, pcap, oncap, K).total; };
             while (total() > lim && pcap > 2048) pcap -= 256;
             while (total() > lim && oncap > 6144) oncap -= 512;
