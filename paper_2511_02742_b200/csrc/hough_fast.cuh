@@ -168,6 +168,18 @@ __device__ __forceinline__ uint32_t fentry_at(const DevParams& P, const uint16_t
 
 // ---------------------------------------------------------------- the fast event kernel
 
+// One vote-count histogram update per distinct count in the warp (peaks of an event share a handful of counts, and
+// same-address shared-memory atomics serialise).  Every lane of the warp must call.
+__device__ __forceinline__ void hist_add(int* hist, bool pk, uint32_t c)
+{
+    const unsigned pm = __ballot_sync(0xffffffffu, pk);
+    if (pk) {
+        const uint32_t cb = min(c, 255u);
+        const unsigned same = __match_any_sync(pm, cb);
+        if ((int)(threadIdx.x & 31) == __ffs(same) - 1) atomicAdd(&hist[cb], __popc(same));
+    }
+}
+
 template <int G, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* __restrict__ v,
@@ -351,10 +363,13 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 if (!(en & kOnFlag)) return 0u;
                 return tl_nb >= 0 ? (slist[(int)(en & 0x7fffu) - on0] & kCountMax) : (uint32_t)halo_prev[P.n_rho + r_nb];
             };
-            for (int i0 = tid - lane; i0 < n_sl; i0 += nthr) {
-                const int i = i0 + lane;
+            // The strip list is in scan order, so neighbouring entries belong to the same cluster.  Lane l of a warp takes entry
+            // l * W + (warp-trip index): the 32 lanes of a warp work on 32 far-apart bins and do not fight over one root.
+            const int W = (n_sl + 31) >> 5;
+            for (int i0 = tid - lane; i0 < W * 32; i0 += nthr) {
+                const int i = lane * W + (i0 >> 5);
                 bool pk = false;
-                uint32_t c = 0, L = 0;
+                uint32_t c = 0, L = 0, q0 = 0xffffffffu, q1 = 0xffffffffu, me_idx = 0;
                 if (i < n_sl) {
                     const uint32_t ent = slist[i];
                     c = ent & kCountMax;
@@ -366,34 +381,43 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     const uint32_t n1 = fentry_at(P, tile, ihalo_prev, tl - 1, r);
                     const uint32_t n2 = fentry_at(P, tile, ihalo_prev, tl - 1, r - 1);
                     const uint32_t n3 = fentry_at(P, tile, ihalo_prev, tl - 1, r + 1);
-                    // joins with the neighbours of smaller linear index; a join is skipped when other joins already imply it
+                    // joins with the neighbours of smaller linear index; a join is skipped when other joins already imply it.
+                    // At most two partners remain; they go through ONE union call site so that the lanes of a warp stay together.
+                    constexpr uint32_t kNone = 0xffffffffu;
                     if (hoff > 0 || (n1 & kOnFlag)) {
-                        if (hoff == 0) suf_union(parent, me, n1 & 0x7fffu);
-                        if ((n0 & kOnFlag) && !(n2 & kOnFlag)) suf_union(parent, me, n0 & 0x7fffu);
+                        if (hoff == 0) q0 = n1 & 0x7fffu;
+                        if ((n0 & kOnFlag) && !(n2 & kOnFlag)) q1 = n0 & 0x7fffu;
                     } else {
-                        if (n0 & kOnFlag) suf_union(parent, me, n0 & 0x7fffu);
-                        else if (n2 & kOnFlag) suf_union(parent, me, n2 & 0x7fffu);
-                        if (n3 & kOnFlag) suf_union(parent, me, n3 & 0x7fffu);
+                        if (n0 & kOnFlag) q0 = n0 & 0x7fffu;
+                        else if (n2 & kOnFlag) q0 = n2 & 0x7fffu;
+                        if (n3 & kOnFlag) q1 = n3 & 0x7fffu;
                     }
+                    if (q0 == kNone) { q0 = q1; q1 = kNone; }
+                    me_idx = me;
                     if (tl < S - 1 || last_strip) {
-                        pk = ncount(n2, tl - 1, r - 1) < c && ncount(n1, tl - 1, r) < c && ncount(n3, tl - 1, r + 1) < c && ncount(n0, tl, r - 1) < c;
-                        if (pk) {
-                            const bool below = tl + 1 < S && base + tl + 1 < P.n_theta;  // else: beyond the grid (last strip)
-                            const uint32_t n4 = fentry_at(P, tile, ihalo_prev, tl, r + 1);
-                            const uint32_t n5 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r - 1) : 0u;
-                            const uint32_t n6 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r) : 0u;
-                            const uint32_t n7 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r + 1) : 0u;
-                            pk = ncount(n4, tl, r + 1) <= c && ncount(n5, tl + 1, r - 1) <= c && ncount(n6, tl + 1, r) <= c &&
-                                 ncount(n7, tl + 1, r + 1) <= c;
-                        }
+                        const bool below = tl + 1 < S && base + tl + 1 < P.n_theta;  // else: beyond the grid (last strip)
+                        const uint32_t n4 = fentry_at(P, tile, ihalo_prev, tl, r + 1);
+                        const uint32_t n5 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r - 1) : 0u;
+                        const uint32_t n6 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r) : 0u;
+                        const uint32_t n7 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r + 1) : 0u;
+                        // no short-circuit: straight-line predicated code instead of eight divergent exits
+                        pk = (ncount(n2, tl - 1, r - 1) < c) & (ncount(n1, tl - 1, r) < c) & (ncount(n3, tl - 1, r + 1) < c) &
+                             (ncount(n0, tl, r - 1) < c) & (ncount(n4, tl, r + 1) <= c) & (ncount(n5, tl + 1, r - 1) <= c) &
+                             (ncount(n6, tl + 1, r) <= c) & (ncount(n7, tl + 1, r + 1) <= c);
                     }
+                }
+#pragma unroll 1
+                for (int kk = 0; kk < 2; ++kk) {
+                    const uint32_t q = kk ? q1 : q0;
+                    if (q != 0xffffffffu) suf_union(parent, me_idx, q);
+                    if (__ballot_sync(0xffffffffu, q1 != 0xffffffffu) == 0) break;  // warp-uniform
                 }
                 __syncwarp();  // reconverge after the data-dependent union loops
                 const int ip = warp_append(&sh.n_peaks, pk);
                 if (pk) {
                     if (ip < P.fPCAP) { peaks[ip] = ((kCountMax - c) << kLBits) | L; pidx[ip] = (uint16_t)(on0 + i); }
-                    atomicAdd(&hist[min(c, 255u)], 1);
                 }
+                hist_add(hist, pk, c);
             }
             if (strip > 0) {  // deferred row: the last theta row of the previous strip, now that row 0 of this one is known
                 for (int r0 = tid - lane; r0 < P.n_rho; r0 += nthr) {
@@ -417,8 +441,8 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                             peaks[ip] = ((kCountMax - c) << kLBits) | (uint32_t)((base - 1) * P.n_rho + r);
                             pidx[ip] = (uint16_t)(ihalo_prev[r] & 0x7fffu);
                         }
-                        atomicAdd(&hist[min(c, 255u)], 1);
                     }
+                    hist_add(hist, pk, c);
                 }
             }
             if (!last_strip) {  // entries of the last theta row, for the next strip's joins and deferred-row peaks
