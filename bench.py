@@ -309,10 +309,16 @@ def run_ours(args):
         hbm_bytes = n_hits * 8 + (n_events + 1) * 8 + n_events * 4 + float(torch.clamp(n_found, max=plan.K).sum().item()) * 32
         peaks_file = os.path.join(ROOT, "MEASURED_PEAKS.json")
         hbm_peak = json.load(open(peaks_file)).get("hbm_gbs") if os.path.exists(peaks_file) else None
-        roofline = {"bound": "smem_atomic", "kernel": "hough_event_kernel (hough_find_clusters)",
+        sm_max = (clocks.get("sm_max_mhz") or 1965.0) * 1e6
+        # diagnostic second ceiling: a vote needs at least 5 issued instructions (2 IMAD, SHF, LOP3, RED) on 4 schedulers / SM
+        alu_peak = info["n_sm"] * 4 * sm_max / 5.0 * 32
+        roofline = {"bound": "smem_atomic", "kernel": "hough_fast_kernel (hough_find_clusters)" if info["fast_groups"] else
+                    "hough_event_kernel (hough_find_clusters)",
                     "achieved": achieved / 1e9, "peak": peak_ops / 1e9, "unit": "Gatomic/s", "frac": achieved / peak_ops,
-                    "peak_source": "hough_measure_smem_atomic_peak, measured live on this GPU (conflict-free red.shared.add.u32, "
-                                   "%.0f MHz); MEASURED_PEAKS.json has no shared-memory figure" % peak_mhz,
+                    "peak_source": "hough_measure_smem_atomic_peak, measured live on this GPU (nothing but conflict-free "
+                                   "red.shared.add.u32, %.0f MHz); MEASURED_PEAKS.json has no shared-memory figure" % peak_mhz,
+                    "alu_issue": {"peak": alu_peak / 1e9, "unit": "Gvote/s", "frac": achieved / alu_peak,
+                                  "note": "5 issue slots per vote x 4 schedulers x n_sm x sm_max_mhz (DESIGN.md)"},
                     "ms_per_launch": ms_find, "share_of_step": ms_find / (ms_find + ms_assign),
                     "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(wl.name) if n_events == wl.n_events else None,
                     "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / (ms_find * 1e-3) / 1e9,
@@ -349,7 +355,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one hough_event_kernel launch, from the ncu --set full capture under
 # profiles/ (workload name -> bytes); None until a capture of that workload exists.
-TRAFFIC_BYTES_PER_LAUNCH = {}
+TRAFFIC_BYTES_PER_LAUNCH = {"cfg3_100k_events_pileup40": 2643605104}   # profiles/r1_fast_kernel_ncu.md
 
 
 def main():

@@ -153,7 +153,8 @@ int64_t hough_plan_launch_count(const hough_plan_t* plan);
 int hough_plan_debug_counters(hough_plan_t* plan, uint64_t* h_out16, void* stream);
 
 /* Measures the conflict-free shared-memory atomic-add rate of the device (the roofline denominator of the
- * vote kernel): every SM runs `red.shared.add.u32` with lane = bank for about `millis` ms.
+ * vote kernel): every SM runs nothing but `red.shared.add.u32` with lane = bank (addresses fixed in registers) for
+ * about `millis` ms.
  * *ops_per_s receives the rate over the whole chip, *sm_clock_mhz the SM clock seen meanwhile. */
 int hough_measure_smem_atomic_peak(int32_t device, double millis, double* ops_per_s, double* sm_clock_mhz);
 

@@ -611,8 +611,9 @@ hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float*
 
 // ---------------------------------------------------------------- roofline denominator probe
 
-// Conflict-free shared-memory atomic adds: lane = bank, 8 addresses per thread, no other work in the loop.
-__global__ void __launch_bounds__(1024, 2)
+// Conflict-free shared-memory atomic adds and nothing else: lane = bank, 16 fixed addresses per thread in registers
+// (rows differ per thread), alternating the two increments the vote kernel uses (+1 -> ATOMS.POPC.INC, +0x10000 -> ATOMS.ADD).
+__global__ void __launch_bounds__(1024, 1)
 smem_atomic_peak_kernel(int iters, int rows, unsigned long long* cycles, uint32_t* sink)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -620,22 +621,18 @@ smem_atomic_peak_kernel(int iters, int rows, unsigned long long* cycles, uint32_
     const int lane = threadIdx.x & 31;
     for (int i = threadIdx.x; i < rows * 32; i += blockDim.x) w[i] = 0;
     __syncthreads();
-    const uint32_t base = smem_addr(w), span = (uint32_t)rows * 128u;
+    const uint32_t base = smem_addr(w);
     uint32_t x = (blockIdx.x * 1315423911u) ^ (threadIdx.x * 2654435761u) ^ 0x9E3779B9u;
-    uint32_t a[8];
+    uint32_t a[16];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < 16; ++j) {
         x = x * 1664525u + 1013904223u;
         a[j] = base + (((x >> 8) % (uint32_t)rows) * 32u + lane) * 4u;
     }
     const long long t0 = clock64();
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            red_add_shared(a[j], 1u);
-            a[j] += 128u * 7u;
-            if (a[j] >= base + span) a[j] -= span;
-        }
+        for (int j = 0; j < 16; ++j) asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a[j]), "r"((j & 1) ? 0x10000u : 1u));
     }
     const long long t1 = clock64();
     __syncthreads();

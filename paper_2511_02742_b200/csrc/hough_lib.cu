@@ -633,7 +633,7 @@ int hough_measure_smem_atomic_peak(int32_t device, double millis, double* ops_pe
     HCK(cudaSetDevice(device));
     cudaDeviceProp prop;
     HCK(cudaGetDeviceProperties(&prop, device));
-    const int threads = 1024, cps = 2, rows = 256;
+    const int threads = 1024, cps = 1, rows = 256;  // one 1024-thread CTA per SM already saturates the unit (32 lanes / clk / SM)
     const int grid = prop.multiProcessorCount * cps;
     const size_t sm = (size_t)rows * 128;
     unsigned long long* d_cyc = nullptr;
@@ -662,7 +662,7 @@ int hough_measure_smem_atomic_peak(int32_t device, double millis, double* ops_pe
     double avg = 0;
     for (int i = 0; i < grid; ++i) avg += (double)cyc[i];
     avg /= grid;
-    *ops_per_s = (double)iters * 8.0 * threads * grid / (ms * 1e-3);
+    *ops_per_s = (double)iters * 16.0 * threads * grid / (ms * 1e-3);
     if (sm_clock_mhz) *sm_clock_mhz = avg / (ms * 1e-3) / 1e6;
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(d_cyc); cudaFree(d_sink);
