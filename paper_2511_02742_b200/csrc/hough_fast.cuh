@@ -38,6 +38,7 @@ struct FastShared {  // static shared control block
     int n_kept, n_ties;
     int defer;
     int cstar, n_gt;  // threshold vote count and number of peaks above it
+    unsigned int r2max;  // max over the event's valid hits of u_q^2 + v_q^2
 };
 
 __device__ __forceinline__ unsigned lanemask_lt()
@@ -111,28 +112,27 @@ template <int G>
 __device__ __forceinline__ void fast_vote(const int2* __restrict__ hits, int n, int sh, uint32_t amask, int Oq2,
                                           const uint32_t (&col)[G], const int (&C)[G][2], const int (&Sn)[G][2])
 {
+    // Hits are sliced over warps two at a time (one 16-byte broadcast load); the next pair is loaded before the current
+    // one is voted, so the load latency hides behind 4 G votes.
     const int warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int4* h4 = reinterpret_cast<const int4*>(hits);
     const int npairs = n >> 1;
-    int i = warp;
-#pragma unroll 1
-    for (; i + nwarps < npairs; i += 2 * nwarps) {  // four hits per trip: two 16-byte broadcast loads
-        const int4 h0 = h4[i];
-        const int4 h1 = h4[i + nwarps];
-        HOUGH_VOTE1(h0.x, h0.y)
-        HOUGH_VOTE1(h0.z, h0.w)
-        HOUGH_VOTE1(h1.x, h1.y)
-        HOUGH_VOTE1(h1.z, h1.w)
-    }
-    if (i < npairs) {
-        const int4 h0 = h4[i];
-        HOUGH_VOTE1(h0.x, h0.y)
-        HOUGH_VOTE1(h0.z, h0.w)
-    }
-    if ((n & 1) && warp == nwarps - 1) {
+    if ((n & 1) && warp == nwarps - 1) {  // odd last hit
         const int2 h = hits[n - 1];
         HOUGH_VOTE1(h.x, h.y)
     }
+    int i = warp;
+    if (i >= npairs) return;
+    int4 cur = h4[i];
+#pragma unroll 1
+    for (i += nwarps; i < npairs; i += nwarps) {
+        const int4 nxt = h4[i];
+        HOUGH_VOTE1(cur.x, cur.y)
+        HOUGH_VOTE1(cur.z, cur.w)
+        cur = nxt;
+    }
+    HOUGH_VOTE1(cur.x, cur.y)
+    HOUGH_VOTE1(cur.z, cur.w)
 }
 #undef HOUGH_VOTE1
 
@@ -209,14 +209,20 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
     const uint32_t tile_base = smem_addr(tile);
     const int k = P.fk, sh_amt = P.fsh, S = P.fS;
-    const uint32_t amask = ~((1u << k) - 1u);
+    uint32_t amask = ~((1u << k) - 1u);
+    int sh_reg = sh_amt;
+    asm volatile("" : "+r"(amask), "+r"(sh_reg));  // per-thread registers (not uniform-datapath operands) for the vote loop
     const int Oq2 = P.Oq + (int)(tile_base << sh_amt);
     uint32_t col[G];
 #pragma unroll
-    for (int g = 0; g < G; ++g) col[g] = 4u * lane + 128u * g;
-    const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe, P.fHB};
+    for (int g = 0; g < G; ++g) {
+        col[g] = 4u * lane + 128u * g;
+        asm volatile("" : "+r"(col[g]));  // one register per column: ((a >> sh) & mask) | col stays a single LOP3 per vote
+    }
+    const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe, P.fHB, &sh.r2max};
     const uint32_t T = (uint32_t)P.T;
     const uint32_t tadd = (0x8000u - T) * 0x00010001u;
+    const uint32_t oadd = (0x8000u - (kCountMax + 1u)) * 0x00010001u;
     const int cpr = 8 * G;  // 16-byte chunks per rho row
 #ifdef HOUGH_PHASE_TIMERS
     long long pt_acc[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -250,10 +256,12 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             reinterpret_cast<uint32_t*>(halo)[P.n_rho + i] = 0;
             reinterpret_cast<uint32_t*>(ihalo)[i] = 0;
         }
-        const int r_lo = 0, r_hi = P.n_rho - 1;
+        if (tid == 0) sh.r2max = 0u;
         for (int i = tid; i < 256; i += nthr) hist[i] = 0;
+        __syncthreads();
         stage_hits(P, sc, u, v, g0, ne);
         HOUGH_PT(0);
+        int r_lo = 0, r_hi = P.n_rho - 1;  // rho rows some vote of this event can reach (set after the first strip's barrier)
 
         bool give_up = false;
         for (int strip = 0; strip < P.f_nstrips; ++strip) {
@@ -264,10 +272,11 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             uint16_t* ihalo_cur = ihalo + (strip & 1) * P.n_rho;
             const uint16_t* halo_prev = halo + ((strip + 1) & 1) * 2 * P.n_rho;
             uint16_t* halo_cur = halo + (strip & 1) * 2 * P.n_rho;
-            {
+            {   // strip 0 clears the whole tile (rows outside [r_lo, r_hi] then stay clear for the event), later strips the
+                // reachable rows plus one on each side (the neighbourhood tests read them)
                 uint4* t4 = reinterpret_cast<uint4*>(tile);
-                const int n16 = P.f_tile_bytes >> 4;
-                for (int i = tid; i < n16; i += nthr) t4[i] = make_uint4(0, 0, 0, 0);
+                const int z_lo = strip == 0 ? 0 : max(r_lo - 1, 0) * cpr, z_hi = strip == 0 ? (P.f_tile_bytes >> 4) : min(r_hi + 2, P.n_rho) * cpr;
+                for (int i = z_lo + tid; i < z_hi; i += nthr) t4[i] = make_uint4(0, 0, 0, 0);
             }
             int C[G][2], Sn[G][2];
             unsigned valid_bits = 0;
@@ -281,10 +290,17 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     if (base + tl < P.n_theta) valid_bits |= 1u << (2 * g + j);
                 }
             __syncthreads();  // tile zeroed, hits staged
+            if (strip == 0) {
+                // |u_q C + v_q S| <= (M + 1) sqrt(u_q^2 + v_q^2) for every theta (Cauchy-Schwarz; the table entries are within 1/2 of
+                // M cos, M sin), so all votes of the event fall into rows [(O_q - B) >> F, (O_q + B) >> F]
+                const long long B = (long long)P.Mq1 * ((long long)ceil(sqrt((double)sh.r2max)) + 1);
+                r_lo = (int)max(((long long)P.Oq - B) >> P.F, 0ll);
+                r_hi = (int)min(((long long)P.Oq + B) >> P.F, (long long)P.n_rho - 1);
+            }
             HOUGH_PT(1);
             {
                 const int ns = sh.n_safe, nu = sh.n_unsafe;
-                if (full) fast_vote<G>(hits, ns, sh_amt, amask, Oq2, col, C, Sn);
+                if (full) fast_vote<G>(hits, ns, sh_reg, amask, Oq2, col, C, Sn);
                 else checked_vote<G>(P, hits, 0, ns, tile_base, k, col, C, Sn, valid_bits);
                 if (nu) checked_vote<G>(P, hits, P.fHB - nu, nu, tile_base, k, col, C, Sn, valid_bits);
             }
@@ -305,9 +321,12 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                         // halfwords sets their top bits exactly where count >= T, without a carry between them
                         const uint32_t gx = (w.x + tadd) & 0x80008000u, gy = (w.y + tadd) & 0x80008000u;
                         const uint32_t gz = (w.z + tadd) & 0x80008000u, gw = (w.w + tadd) & 0x80008000u;
-                        if (gx | gy | gz | gw)
+                        if (gx | gy | gz | gw) {
                             m = (((gx >> 15) | (gx >> 30)) & 3u) | ((((gy >> 15) | (gy >> 30)) & 3u) << 2) |
                                 ((((gz >> 15) | (gz >> 30)) & 3u) << 4) | ((((gw >> 15) | (gw >> 30)) & 3u) << 6);
+                            // a count above 1023 does not fit the packed entries: the general kernel takes the event
+                            if (((w.x + oadd) | (w.y + oadd) | (w.z + oadd) | (w.w + oadd)) & 0x80008000u) sh.defer = 1;
+                        }
                         // theta rows beyond n_theta hold no votes (checked_vote masks them), so m needs no masking
                     }
                     if (__ballot_sync(0xffffffffu, m != 0) == 0) continue;
@@ -319,18 +338,15 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     if (lane == 31) wbase = atomicAdd(&sh.n_sl, incl);
                     wbase = __shfl_sync(0xffffffffu, wbase, 31);
                     int slot = wbase + incl - cnt;
-                    const int r = idx >> (k - 4), tl0 = (idx & (cpr - 1)) * 8;  // cpr = 2^(k-4) chunks per row
-                    const uint32_t heads = m & ~(m << 1);  // first bin of every run of consecutive theta rows in this chunk
+                    // chunk idx holds the tile halfwords 8 idx ... 8 idx + 7 (rows are 8 cpr halfwords long)
+                    const uint32_t above = m << 1;  // bit q set <=> the bin one theta row up, in this chunk, is on
+                    const uint32_t loc0 = (uint32_t)idx << 3;
                     while (m) {
                         const int q = __ffs(m) - 1;
                         m &= m - 1;
-                        const uint32_t wq = (q < 4) ? ((q < 2) ? w.x : w.y) : ((q < 6) ? w.z : w.w);
-                        const uint32_t c = (wq >> (16 * (q & 1))) & 0xffffu;
-                        if (c > kCountMax) sh.defer = 1;
-                        const int hoff = q - (31 - __clz(heads & ((2u << q) - 1u)));  // distance to the head of its run (0..7)
-                        // strip-list entry: run-head distance (3 bits) | bin index inside the tile (17 bits) | votes (10 bits)
+                        // strip-list entry: "joins the entry before it" (bit 27) | bin index inside the tile (17 bits) | votes (10 bits)
                         if (slot < P.fSLCAP)
-                            slist[slot] = ((uint32_t)hoff << 27) | ((uint32_t)(r * S + tl0 + q) << kCountBits) | (c & kCountMax);
+                            slist[slot] = (((above >> q) & 1u) << 27) | ((loc0 + q) << kCountBits) | ((uint32_t)tile[loc0 + q] & kCountMax);
                         ++slot;
                     }
                 }
@@ -351,7 +367,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             for (int i = tid; i < n_sl; i += nthr) {
                 const uint32_t ent = slist[i];
                 tile[(ent >> kCountBits) & 0x1ffffu] = (uint16_t)(kOnFlag | (uint32_t)(on0 + i));
-                parent[on0 + i] = (unsigned short)(on0 + i - (int)(ent >> 27));
+                parent[on0 + i] = (unsigned short)(on0 + i - (int)(ent >> 27));  // bit 27: joins the entry before it
             }
             __syncthreads();
             HOUGH_PT(5);

@@ -57,6 +57,7 @@ struct DevParams {
     // ---- fast path (hough_fast.cuh); f_enabled == 0 when the plan cannot use it
     int f_enabled;
     int rho_shift;                   // log2(n_rho) if n_rho is a power of two, else -1
+    int Mq1;                         // ceil(M) + 1 >= max over theta of sqrt(C_q^2 + S_q^2)
     int fk, fsh;                     // log2(row bytes), F - fk
     int fS, f_nstrips, f_tile_bytes; // theta rows per strip (64 G), strips per event
     int fHB, fSLCAP, fPCAP;          // capacities: staged hits, strip list, peak list
@@ -124,15 +125,17 @@ struct StageCtx {
     int* n_safe;  // shared counters
     int* n_unsafe;
     int hb;
+    unsigned int* r2max;  // nullable: max of u_q^2 + v_q^2 over the valid hits (shared)
 };
 
-__device__ __forceinline__ void stage_one(const DevParams& P, const StageCtx& sc, float u, float v)
+__device__ __forceinline__ void stage_one(const DevParams& P, const StageCtx& sc, float u, float v, unsigned int& r2loc)
 {
     // valid <=> finite and |u|, |v| <= coord_max  (NaN fails the comparison, Inf exceeds coord_max)
     if (!(fabsf(u) <= P.coord_max) || !(fabsf(v) <= P.coord_max)) return;
     const int uq = __float2int_rn(u * P.hit_scale);  // exact product (power-of-two scale), ties to even
     const int vq = __float2int_rn(v * P.hit_scale);
     const unsigned long long r2 = (unsigned long long)((long long)uq * uq) + (unsigned long long)((long long)vq * vq);
+    r2loc = max(r2loc, r2 > 0xffffffffull ? 0xffffffffu : (unsigned int)r2);
     if (P.safe_enabled && r2 <= P.r2safe) {
         sc.hits[atomicAdd(sc.n_safe, 1)] = make_int2(uq, vq);
     } else {
@@ -146,20 +149,22 @@ __device__ __forceinline__ void stage_hits(const DevParams& P, const StageCtx& s
 {
     const long long a0 = g0 & ~3LL;
     const long long g1 = g0 + n;
+    unsigned int r2loc = 0;
     for (long long i = a0 + 4LL * threadIdx.x; i < g1; i += 4LL * blockDim.x) {
         if (i >= g0 && i + 4 <= g1) {
             const float4 uu = __ldg(reinterpret_cast<const float4*>(u + i));
             const float4 vv = __ldg(reinterpret_cast<const float4*>(v + i));
-            stage_one(P, sc, uu.x, vv.x);
-            stage_one(P, sc, uu.y, vv.y);
-            stage_one(P, sc, uu.z, vv.z);
-            stage_one(P, sc, uu.w, vv.w);
+            stage_one(P, sc, uu.x, vv.x, r2loc);
+            stage_one(P, sc, uu.y, vv.y, r2loc);
+            stage_one(P, sc, uu.z, vv.z, r2loc);
+            stage_one(P, sc, uu.w, vv.w, r2loc);
         } else {
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-                if (i + j >= g0 && i + j < g1) stage_one(P, sc, __ldg(u + i + j), __ldg(v + i + j));
+                if (i + j >= g0 && i + j < g1) stage_one(P, sc, __ldg(u + i + j), __ldg(v + i + j), r2loc);
         }
     }
+    if (sc.r2max && r2loc) atomicMax(sc.r2max, r2loc);
 }
 
 // ---------------------------------------------------------------- S1: voting
@@ -264,7 +269,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
     const uint32_t colbase = smem_addr(tile) + 4u * lane;
-    const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe, P.HB};
+    const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe, P.HB, nullptr};
 
     uint32_t* parent = P.parent + (size_t)blockIdx.x * P.n_bins;
     uint32_t* csize = P.csize + (size_t)blockIdx.x * P.n_bins;

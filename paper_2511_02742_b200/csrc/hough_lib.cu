@@ -440,6 +440,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     P.f_work_counter = p->d_counter + 1;
     P.deferred_count = p->d_counter + 2;
     P.f_enabled = p->f_G != 0;
+    P.Mq1 = (int)ceil(M) + 1;
     P.rho_shift = -1;
     for (int b = 0; b < 31; ++b) if ((1 << b) == d->n_rho) P.rho_shift = b;
     if (p->f_G) {
