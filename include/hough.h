@@ -132,9 +132,11 @@ int hough_assign_hits(hough_plan_t* plan, const float* d_u, const float* d_v, co
 
 /* ---- helpers beyond the five ---- */
 
-/* hough_find_clusters + hough_assign_hits on HOST buffers: copies u, v, offsets to the device, runs both
- * kernels, copies cands, n_found and labels back, and synchronises.  h_offsets[0] must be 0 and
- * h_offsets[n_events] the number of hits.  Any output pointer may be NULL (then it is not copied back). */
+/* hough_find_clusters + hough_assign_hits on HOST buffers (pinned memory makes the copies asynchronous): the batch is cut
+ * into chunks of events; a chunk's hits are copied to the device while the previous chunk is computed and the one before
+ * that is copied back (three internal streams), then the call synchronises.  h_offsets[0] must be 0, h_offsets must be
+ * non-decreasing and h_offsets[n_events] the number of hits.  Any output pointer may be NULL (then it is not copied
+ * back); records beyond min(n_found, K) of an event are zero on the first call and otherwise unspecified. */
 int hough_run_host(hough_plan_t* plan, const float* h_u, const float* h_v, const int64_t* h_offsets,
                    int32_t n_events, hough_candidate_t* h_cands, int32_t* h_n_found, int32_t* h_labels);
 

@@ -33,6 +33,8 @@ static int cuda_fail(cudaError_t e, const char* what)
         if (e_ != cudaSuccess) return cuda_fail(e_, #call);         \
     } while (0)
 
+static const int kHostChunksMax = 32;
+
 struct hough_plan {
     hough_plan_desc_t desc;
     DevParams P;
@@ -54,7 +56,9 @@ struct hough_plan {
     int* d_status;
     unsigned int* d_counter;
     // lazily created resources of hough_run_host
-    cudaStream_t h_stream;
+    cudaStream_t h_stream;               // compute stream of hough_run_host
+    cudaStream_t h_up, h_down;           // copy streams: host -> device, device -> host
+    cudaEvent_t h_ev_up[kHostChunksMax], h_ev_done[kHostChunksMax];
     float* hd_u;
     float* hd_v;
     long long* hd_off;
@@ -473,7 +477,15 @@ int hough_plan_destroy(hough_plan_t* p)
     cudaFree(p->d_cos); cudaFree(p->d_sin); cudaFree(p->d_scratch); cudaFree(p->d_status);
     cudaFree(p->d_fcos); cudaFree(p->d_fsin); cudaFree(p->d_deferred);
     cudaFree(p->hd_u); cudaFree(p->hd_v); cudaFree(p->hd_off); cudaFree(p->hd_cands); cudaFree(p->hd_nfound); cudaFree(p->hd_labels);
-    if (p->h_stream) cudaStreamDestroy(p->h_stream);
+    if (p->h_stream) {
+        cudaStreamDestroy(p->h_stream);
+        if (p->h_up) cudaStreamDestroy(p->h_up);
+        if (p->h_down) cudaStreamDestroy(p->h_down);
+        for (int c = 0; c < kHostChunksMax; ++c) {
+            if (p->h_ev_up[c]) cudaEventDestroy(p->h_ev_up[c]);
+            if (p->h_ev_done[c]) cudaEventDestroy(p->h_ev_done[c]);
+        }
+    }
     (void)cudaGetLastError();
     delete p;
     return HOUGH_OK;
@@ -600,30 +612,69 @@ int hough_run_host(hough_plan_t* p, const float* h_u, const float* h_v, const in
     if (!p->h_stream) {
         const size_t mh = (size_t)(p->desc.max_hits > 0 ? p->desc.max_hits : 1) + 4, me = (size_t)p->desc.max_events;
         HCK(cudaStreamCreateWithFlags(&p->h_stream, cudaStreamNonBlocking));
+        HCK(cudaStreamCreateWithFlags(&p->h_up, cudaStreamNonBlocking));
+        HCK(cudaStreamCreateWithFlags(&p->h_down, cudaStreamNonBlocking));
+        for (int c = 0; c < kHostChunksMax; ++c) {
+            HCK(cudaEventCreateWithFlags(&p->h_ev_up[c], cudaEventDisableTiming));
+            HCK(cudaEventCreateWithFlags(&p->h_ev_done[c], cudaEventDisableTiming));
+        }
         HCK(cudaMalloc((void**)&p->hd_u, mh * 4));
         HCK(cudaMalloc((void**)&p->hd_v, mh * 4));
         HCK(cudaMalloc((void**)&p->hd_off, (me + 1) * 8));
         HCK(cudaMalloc((void**)&p->hd_cands, me * p->desc.max_candidates * sizeof(Candidate)));
         HCK(cudaMalloc((void**)&p->hd_nfound, me * 4));
         HCK(cudaMalloc((void**)&p->hd_labels, mh * 4));
+        HCK(cudaMemset(p->hd_cands, 0, me * p->desc.max_candidates * sizeof(Candidate)));  // rows beyond n_found read as zeros
     }
+    // The batch is cut into chunks of events with about equal hit counts; chunk c's hits go up on one stream while chunk
+    // c - 1 is computed on a second and chunk c - 2's results come down on a third (PCIe is full duplex).  The kernels of all
+    // chunks run on ONE stream, in order: the plan's counters and scratch are not shared between concurrent launches.
+    int n_chunks = env_int("HOUGH_HOST_CHUNKS", 0);
+    if (n_chunks <= 0) n_chunks = (int)(n_hits / (24ll << 20)) + 1;  // ~24 M hits (200 MB of input) per chunk
+    if (n_chunks > kHostChunksMax) n_chunks = kHostChunksMax;
+    if (n_chunks > n_events) n_chunks = n_events;
+    const size_t K = (size_t)p->desc.max_candidates;
     cudaStream_t st = p->h_stream;
-    HCK(cudaMemcpyAsync(p->hd_off, h_offsets, (size_t)(n_events + 1) * 8, cudaMemcpyHostToDevice, st));
-    if (n_hits > 0) {
-        HCK(cudaMemcpyAsync(p->hd_u, h_u, (size_t)n_hits * 4, cudaMemcpyHostToDevice, st));
-        HCK(cudaMemcpyAsync(p->hd_v, h_v, (size_t)n_hits * 4, cudaMemcpyHostToDevice, st));
+    HCK(cudaMemcpyAsync(p->hd_off, h_offsets, (size_t)(n_events + 1) * 8, cudaMemcpyHostToDevice, p->h_up));
+    int e0 = 0;
+    for (int c = 0; c < n_chunks; ++c) {
+        int e1 = n_events;
+        if (c + 1 < n_chunks) {  // first event boundary at or after the c + 1-th share of the hits
+            const int64_t target = n_hits / n_chunks * (c + 1);
+            int lo = e0, hi = n_events;
+            while (lo < hi) { const int mid = (lo + hi) / 2; if (h_offsets[mid] < target) lo = mid + 1; else hi = mid; }
+            e1 = lo < e0 ? e0 : lo;
+        }
+        const int ne = e1 - e0;
+        const int64_t a = h_offsets[e0], z = h_offsets[e1];
+        if (z < a || a < 0 || z > n_hits) return HOUGH_EINVAL;  // offsets must be non-decreasing on this path
+        if (z > a) {
+            HCK(cudaMemcpyAsync(p->hd_u + a, h_u + a, (size_t)(z - a) * 4, cudaMemcpyHostToDevice, p->h_up));
+            HCK(cudaMemcpyAsync(p->hd_v + a, h_v + a, (size_t)(z - a) * 4, cudaMemcpyHostToDevice, p->h_up));
+        }
+        HCK(cudaEventRecord(p->h_ev_up[c], p->h_up));
+        HCK(cudaStreamWaitEvent(st, p->h_ev_up[c], 0));
+        if (ne > 0) {
+            int rc = hough_find_clusters(p, p->hd_u, p->hd_v, reinterpret_cast<const int64_t*>(p->hd_off) + e0, ne,
+                                         reinterpret_cast<hough_candidate_t*>(p->hd_cands) + (size_t)e0 * K, p->hd_nfound + e0, st);
+            if (rc) return rc;
+            if (h_labels) {
+                rc = hough_assign_hits(p, p->hd_u, p->hd_v, reinterpret_cast<const int64_t*>(p->hd_off) + e0, ne,
+                                       reinterpret_cast<const hough_candidate_t*>(p->hd_cands) + (size_t)e0 * K, p->hd_nfound + e0,
+                                       p->hd_labels, st);
+                if (rc) return rc;
+            }
+        }
+        HCK(cudaEventRecord(p->h_ev_done[c], st));
+        HCK(cudaStreamWaitEvent(p->h_down, p->h_ev_done[c], 0));
+        if (ne > 0) {
+            if (h_labels && z > a) HCK(cudaMemcpyAsync(h_labels + a, p->hd_labels + a, (size_t)(z - a) * 4, cudaMemcpyDeviceToHost, p->h_down));
+            if (h_cands) HCK(cudaMemcpyAsync(h_cands + (size_t)e0 * K, p->hd_cands + (size_t)e0 * K, (size_t)ne * K * sizeof(Candidate), cudaMemcpyDeviceToHost, p->h_down));
+            if (h_n_found) HCK(cudaMemcpyAsync(h_n_found + e0, p->hd_nfound + e0, (size_t)ne * 4, cudaMemcpyDeviceToHost, p->h_down));
+        }
+        e0 = e1;
     }
-    int rc = hough_find_clusters(p, p->hd_u, p->hd_v, reinterpret_cast<const int64_t*>(p->hd_off), n_events,
-                                 reinterpret_cast<hough_candidate_t*>(p->hd_cands), p->hd_nfound, st);
-    if (rc) return rc;
-    if (h_labels) {
-        rc = hough_assign_hits(p, p->hd_u, p->hd_v, reinterpret_cast<const int64_t*>(p->hd_off), n_events,
-                               reinterpret_cast<const hough_candidate_t*>(p->hd_cands), p->hd_nfound, p->hd_labels, st);
-        if (rc) return rc;
-        if (n_hits > 0) HCK(cudaMemcpyAsync(h_labels, p->hd_labels, (size_t)n_hits * 4, cudaMemcpyDeviceToHost, st));
-    }
-    if (h_cands) HCK(cudaMemcpyAsync(h_cands, p->hd_cands, (size_t)n_events * p->desc.max_candidates * sizeof(Candidate), cudaMemcpyDeviceToHost, st));
-    if (h_n_found) HCK(cudaMemcpyAsync(h_n_found, p->hd_nfound, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st));
+    HCK(cudaStreamSynchronize(p->h_down));
     HCK(cudaStreamSynchronize(st));
     return HOUGH_OK;
 }
