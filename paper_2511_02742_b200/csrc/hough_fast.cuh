@@ -108,31 +108,38 @@ __device__ __forceinline__ void suf_union(unsigned short* parent, uint32_t a, ui
         }                                                                                                \
     }
 
-template <int G>
+template <int G, int NW>
 __device__ __forceinline__ void fast_vote(const int2* __restrict__ hits, int n, int sh, uint32_t amask, int Oq2,
                                           const uint32_t (&col)[G], const int (&C)[G][2], const int (&Sn)[G][2])
 {
-    // Hits are sliced over warps two at a time (one 16-byte broadcast load); the next pair is loaded before the current
-    // one is voted, so the load latency hides behind 4 G votes.
-    const int warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const int4* h4 = reinterpret_cast<const int4*>(hits);
+    // Hits are sliced over the NW warps of the CTA two at a time (one 16-byte broadcast load); a trip takes four such
+    // pairs (the loads carry their strides as immediates), so the loop overhead is 7 instructions per 32 G votes.
+    const int warp = threadIdx.x >> 5;
     const int npairs = n >> 1;
-    if ((n & 1) && warp == nwarps - 1) {  // odd last hit
+    if ((n & 1) && warp == NW - 1) {  // odd last hit
         const int2 h = hits[n - 1];
         HOUGH_VOTE1(h.x, h.y)
     }
+    const int4* p = reinterpret_cast<const int4*>(hits) + warp;
     int i = warp;
-    if (i >= npairs) return;
-    int4 cur = h4[i];
 #pragma unroll 1
-    for (i += nwarps; i < npairs; i += nwarps) {
-        const int4 nxt = h4[i];
-        HOUGH_VOTE1(cur.x, cur.y)
-        HOUGH_VOTE1(cur.z, cur.w)
-        cur = nxt;
+    for (; i + 3 * NW < npairs; i += 4 * NW, p += 4 * NW) {
+        const int4 h0 = p[0], h1 = p[NW], h2 = p[2 * NW], h3 = p[3 * NW];
+        HOUGH_VOTE1(h0.x, h0.y)
+        HOUGH_VOTE1(h0.z, h0.w)
+        HOUGH_VOTE1(h1.x, h1.y)
+        HOUGH_VOTE1(h1.z, h1.w)
+        HOUGH_VOTE1(h2.x, h2.y)
+        HOUGH_VOTE1(h2.z, h2.w)
+        HOUGH_VOTE1(h3.x, h3.y)
+        HOUGH_VOTE1(h3.z, h3.w)
     }
-    HOUGH_VOTE1(cur.x, cur.y)
-    HOUGH_VOTE1(cur.z, cur.w)
+#pragma unroll 1
+    for (; i < npairs; i += NW, p += NW) {
+        const int4 h0 = p[0];
+        HOUGH_VOTE1(h0.x, h0.y)
+        HOUGH_VOTE1(h0.z, h0.w)
+    }
 }
 #undef HOUGH_VOTE1
 
@@ -214,11 +221,11 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
     asm volatile("" : "+r"(amask), "+r"(sh_reg));  // per-thread registers (not uniform-datapath operands) for the vote loop
     const int Oq2 = P.Oq + (int)(tile_base << sh_amt);
     uint32_t col[G];
+    // 128 bytes between a lane's word columns, taken from a kernel parameter (2 fS / G with fS = 64 G): ptxas cannot
+    // fold col[g] back into col[0] | constant, so ((a >> sh) & mask) | col[g] stays ONE LOP3 per vote for every g
+    const uint32_t col_stride = (uint32_t)(2 * P.fS) / (uint32_t)G;
 #pragma unroll
-    for (int g = 0; g < G; ++g) {
-        col[g] = 4u * lane + 128u * g;
-        asm volatile("" : "+r"(col[g]));  // one register per column: ((a >> sh) & mask) | col stays a single LOP3 per vote
-    }
+    for (int g = 0; g < G; ++g) col[g] = 4u * lane + col_stride * g;
     const StageCtx sc{hits, &sh.n_safe, &sh.n_unsafe, P.fHB, &sh.r2max};
     const uint32_t T = (uint32_t)P.T;
     const uint32_t tadd = (0x8000u - T) * 0x00010001u;
@@ -300,7 +307,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             HOUGH_PT(1);
             {
                 const int ns = sh.n_safe, nu = sh.n_unsafe;
-                if (full) fast_vote<G>(hits, ns, sh_reg, amask, Oq2, col, C, Sn);
+                if (full) fast_vote<G, MAXT / 32>(hits, ns, sh_reg, amask, Oq2, col, C, Sn);  // launched with MAXT threads
                 else checked_vote<G>(P, hits, 0, ns, tile_base, k, col, C, Sn, valid_bits);
                 if (nu) checked_vote<G>(P, hits, P.fHB - nu, nu, tile_base, k, col, C, Sn, valid_bits);
             }
@@ -425,7 +432,9 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 #pragma unroll 1
                 for (int kk = 0; kk < 2; ++kk) {
                     const uint32_t q = kk ? q1 : q0;
+#if !defined(HOUGH_EXP) || HOUGH_EXP != 1
                     if (q != 0xffffffffu) suf_union(parent, me_idx, q);
+#endif
                     if (__ballot_sync(0xffffffffu, q1 != 0xffffffffu) == 0) break;  // warp-uniform
                 }
                 __syncwarp();  // reconverge after the data-dependent union loops
@@ -435,6 +444,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 }
                 hist_add(hist, pk, c);
             }
+            HOUGH_PT(2);
             if (strip > 0) {  // deferred row: the last theta row of the previous strip, now that row 0 of this one is known
                 for (int r0 = tid - lane; r0 < P.n_rho; r0 += nthr) {
                     const int r = r0 + lane;
@@ -461,6 +471,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     hist_add(hist, pk, c);
                 }
             }
+            HOUGH_PT(9);
             if (!last_strip) {  // entries of the last theta row, for the next strip's joins and deferred-row peaks
                 for (int r = tid; r < P.n_rho; r += nthr) {
                     const uint16_t en = tile[r * S + S - 1];

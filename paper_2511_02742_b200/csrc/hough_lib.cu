@@ -330,9 +330,8 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
         // preference order: one 1024-thread CTA per SM with the widest tile row that fits, then two CTAs per SM
         const Cand cands[] = {{4, 1024, 1, 1024, 1}, {2, 1024, 1, 1024, 1}, {1, 1024, 1, 1024, 1}, {4, 768, 2, 768, 2}, {2, 768, 2, 768, 2}, {1, 768, 2, 768, 2}};
         const int want_G = env_int("HOUGH_FAST_G", 0), want_t = env_int("HOUGH_FAST_MAXT", 0), want_b = env_int("HOUGH_FAST_MINB", 0);
-        const int want_threads = env_int("HOUGH_FAST_THREADS", 0);
         std::vector<Cand> list(cands, cands + sizeof(cands) / sizeof(cands[0]));
-        if (want_G && want_t && want_b) list.assign(1, Cand{want_G, want_t, want_b, want_threads > 0 ? want_threads : want_t, want_b});
+        if (want_G && want_t && want_b) list.assign(1, Cand{want_G, want_t, want_b, want_t, want_b}  /* the kernel assumes blockDim.x == MAXT */);
         for (const Cand& c : list) {
             const int rows = 64 * c.G;
             if (rows > 64 && rows / 2 >= d->n_theta) continue;  // a narrower tile already covers every theta row
