@@ -32,6 +32,7 @@ constexpr uint32_t kCountMax = (1u << kCountBits) - 1;
 struct FastShared {  // static shared control block
     int event;
     int n_safe, n_unsafe;
+    int n_ch;     // on chunks of the current strip (grow down from the end of the strip list)
     int n_sl;     // on bins of the current strip (strip list)
     int n_on;     // on bins of the event so far (global on list)
     int n_peaks;  // peaks of the event so far
@@ -240,7 +241,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
         __syncthreads();  // previous event fully done
         if (tid == 0) {
             sh.event = (int)atomicAdd(P.f_work_counter, 1u);
-            sh.n_safe = 0; sh.n_unsafe = 0; sh.n_sl = 0; sh.n_on = 0; sh.n_peaks = 0; sh.n_kept = 0; sh.n_ties = 0; sh.defer = 0;
+            sh.n_safe = 0; sh.n_unsafe = 0; sh.n_ch = 0; sh.n_sl = 0; sh.n_on = 0; sh.n_peaks = 0; sh.n_kept = 0; sh.n_ties = 0; sh.defer = 0;
         }
         __syncthreads();
         const int e = sh.event;
@@ -284,6 +285,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 uint4* t4 = reinterpret_cast<uint4*>(tile);
                 const int z_lo = strip == 0 ? 0 : max(r_lo - 1, 0) * cpr, z_hi = strip == 0 ? (P.f_tile_bytes >> 4) : min(r_hi + 2, P.n_rho) * cpr;
                 for (int i = z_lo + tid; i < z_hi; i += nthr) t4[i] = make_uint4(0, 0, 0, 0);
+                for (int i = tid; i < P.n_rho; i += nthr) ihalo_cur[i] = 0;  // filled by step (b)
             }
             int C[G][2], Sn[G][2];
             unsigned valid_bits = 0;
@@ -314,16 +316,17 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             __syncthreads();  // all votes of the strip are in
             HOUGH_PT(3);
 
-            // ---------------- S2: threshold, compaction of the strip's on bins
+            // ---------------- S2: threshold.  Pass 1 (sparse: one warp trip in two finds nothing) only appends the on CHUNKS
+            // (chunk index | on mask << 16) to a list that grows down from the end of the strip list: one ballot, one atomic
+            // per warp trip.  Pass 2 (dense: one thread per on chunk) expands them into the strip list's per-bin entries.
             {
                 const uint4* t4 = reinterpret_cast<const uint4*>(tile);
                 const int i_lo = r_lo * cpr, i_hi = (r_hi + 1) * cpr;  // only rho rows some hit can reach
                 for (int i0 = i_lo + tid - lane; i0 < i_hi; i0 += nthr) {
                     const int idx = i0 + lane;
                     uint32_t m = 0;  // bit q set <=> count q of this chunk is on
-                    uint4 w = make_uint4(0, 0, 0, 0);
                     if (idx < i_hi) {
-                        w = t4[idx];
+                        const uint4 w = t4[idx];
                         // counts are below 2^15 (at most one vote per hit, fHB <= 32767), so adding 2^15 - T to both
                         // halfwords sets their top bits exactly where count >= T, without a carry between them
                         const uint32_t gx = (w.x + tadd) & 0x80008000u, gy = (w.y + tadd) & 0x80008000u;
@@ -335,79 +338,143 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                             if (((w.x + oadd) | (w.y + oadd) | (w.z + oadd) | (w.w + oadd)) & 0x80008000u) sh.defer = 1;
                         }
                         // theta rows beyond n_theta hold no votes (checked_vote masks them), so m needs no masking
+                        if ((idx & (cpr - 1)) == cpr - 1) {  // last chunk of a rho row: its two last counts are the next strip's halo
+                            const int r = idx / cpr;         // (rows no vote can reach are never scanned: they stay 0 from the event's start)
+                            halo_cur[r] = (uint16_t)(w.w & 0xffffu);
+                            halo_cur[P.n_rho + r] = (uint16_t)(w.w >> 16);
+                        }
                     }
-                    if (__ballot_sync(0xffffffffu, m != 0) == 0) continue;
-                    const int cnt = __popc(m);
-                    int incl = cnt;
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
-                    int wbase = 0;
-                    if (lane == 31) wbase = atomicAdd(&sh.n_sl, incl);
-                    wbase = __shfl_sync(0xffffffffu, wbase, 31);
-                    int slot = wbase + incl - cnt;
-                    // chunk idx holds the tile halfwords 8 idx ... 8 idx + 7 (rows are 8 cpr halfwords long)
-                    const uint32_t above = m << 1;  // bit q set <=> the bin one theta row up, in this chunk, is on
-                    const uint32_t loc0 = (uint32_t)idx << 3;
-                    while (m) {
-                        const int q = __ffs(m) - 1;
-                        m &= m - 1;
-                        // strip-list entry: "joins the entry before it" (bit 27) | bin index inside the tile (17 bits) | votes (10 bits)
-                        if (slot < P.fSLCAP)
-                            slist[slot] = (((above >> q) & 1u) << 27) | ((loc0 + q) << kCountBits) | ((uint32_t)tile[loc0 + q] & kCountMax);
-                        ++slot;
-                    }
+                    const unsigned bal = __ballot_sync(0xffffffffu, m != 0);
+                    if (bal == 0) continue;
+                    int cb = 0;
+                    if (lane == 0) cb = atomicAdd(&sh.n_ch, __popc(bal));
+                    cb = __shfl_sync(0xffffffffu, cb, 0) + __popc(bal & lanemask_lt());
+                    if (m != 0 && cb < P.fSLCAP) slist[P.fSLCAP - 1 - cb] = (uint32_t)idx | (m << 16);
                 }
             }
-            if (!last_strip) {  // counts of the last two theta rows, for the next strip's local-maximum tests
-                for (int r = tid; r < P.n_rho; r += nthr) {
-                    halo_cur[r] = tile[r * S + S - 2];
-                    halo_cur[P.n_rho + r] = tile[r * S + S - 1];
+            __syncthreads();
+            const int n_ch = sh.n_ch;
+            if (sh.defer || n_ch > P.fSLCAP) { give_up = true; break; }  // block-uniform
+            const int sl_lim = P.fSLCAP - n_ch;  // per-bin entries fill [0, sl_lim), the chunk list sits behind them
+            // One thread per on chunk (8 consecutive theta rows of one rho row).  The counts are still intact, so the strict
+            // local-maximum test (O4) is done here for the 8 bins at once on packed halfwords: with a / b / c the counts of rho
+            // rows r-1 / r / r+1 and V[q] = max(a[q], b[q], c[q]),
+            //     peak(q) <=> on(q) and b[q] > max(V[q-1], a[q]) and b[q] >= max(V[q+1], c[q])
+            // (the neighbours of smaller linear index must be beaten, the others matched).  A bin of the strip's last theta
+            // row waits for the next strip ("deferred row" below) unless this is the last strip.
+            for (int j0 = tid - lane; j0 < n_ch; j0 += nthr) {
+                const int j = j0 + lane;
+                uint32_t m = 0, loc0 = 0, pk8 = 0;
+                uint4 Bw = make_uint4(0, 0, 0, 0);
+                if (j < n_ch) {
+                    const uint32_t ce = slist[P.fSLCAP - 1 - j];
+                    m = ce >> 16;
+                    const int cidx = (int)(ce & 0xffffu);
+                    loc0 = (uint32_t)cidx << 3;  // chunk idx holds the tile halfwords 8 idx ... 8 idx + 7
+                    const int r = cidx / cpr, cq = cidx & (cpr - 1);
+                    const bool up = r > 0, dn = r + 1 < P.n_rho;
+                    const uint4* t4 = reinterpret_cast<const uint4*>(tile);
+                    const uint4 z4 = make_uint4(0, 0, 0, 0);
+                    Bw = t4[cidx];
+                    const uint4 Aw = up ? t4[cidx - cpr] : z4, Cw = dn ? t4[cidx + cpr] : z4;
+                    uint32_t em, ep = 0;  // max of the three counts one theta row before / after the chunk
+                    if (cq > 0) {
+                        const uint16_t* e = tile + loc0 - 1;
+                        em = max((uint32_t)e[0], max(up ? (uint32_t)e[-S] : 0u, dn ? (uint32_t)e[S] : 0u));
+                    } else {  // the previous strip's last theta row (all zero for the first strip)
+                        const uint16_t* e = halo_prev + P.n_rho + r;
+                        em = max((uint32_t)e[0], max(up ? (uint32_t)e[-1] : 0u, dn ? (uint32_t)e[1] : 0u));
+                    }
+                    if (cq < cpr - 1) {
+                        const uint16_t* e = tile + loc0 + 8;
+                        ep = max((uint32_t)e[0], max(up ? (uint32_t)e[-S] : 0u, dn ? (uint32_t)e[S] : 0u));
+                    }
+                    const uint32_t V0 = __vmaxu2(__vmaxu2(Aw.x, Bw.x), Cw.x), V1 = __vmaxu2(__vmaxu2(Aw.y, Bw.y), Cw.y);
+                    const uint32_t V2 = __vmaxu2(__vmaxu2(Aw.z, Bw.z), Cw.z), V3 = __vmaxu2(__vmaxu2(Aw.w, Bw.w), Cw.w);
+                    // Vm_j = (V[2j-1], V[2j]): the column maxima one theta row up; one theta row down it is Vm_(j+1)
+                    const uint32_t Vm0 = __byte_perm(em << 16, V0, 0x5432), Vm1 = __byte_perm(V0, V1, 0x5432);
+                    const uint32_t Vm2 = __byte_perm(V1, V2, 0x5432), Vm3 = __byte_perm(V2, V3, 0x5432), Vm4 = __byte_perm(V3, ep, 0x5432);
+                    // counts are below 2^15: (b | 2^15) - x keeps bit 15 exactly where b >= x, without a borrow between the halfwords
+                    auto pkw = [](uint32_t bw, uint32_t sm, uint32_t nm) -> uint32_t {
+                        const uint32_t bh = bw | 0x80008000u;
+                        return (bh - sm - 0x00010001u) & (bh - nm) & 0x80008000u;
+                    };
+                    const uint32_t gx = pkw(Bw.x, __vmaxu2(Vm0, Aw.x), __vmaxu2(Vm1, Cw.x)), gy = pkw(Bw.y, __vmaxu2(Vm1, Aw.y), __vmaxu2(Vm2, Cw.y));
+                    const uint32_t gz = pkw(Bw.z, __vmaxu2(Vm2, Aw.z), __vmaxu2(Vm3, Cw.z)), gw = pkw(Bw.w, __vmaxu2(Vm3, Aw.w), __vmaxu2(Vm4, Cw.w));
+                    pk8 = (((gx >> 15) | (gx >> 30)) & 3u) | ((((gy >> 15) | (gy >> 30)) & 3u) << 2) |
+                          ((((gz >> 15) | (gz >> 30)) & 3u) << 4) | ((((gw >> 15) | (gw >> 30)) & 3u) << 6);
+                    pk8 &= m;
+                    if (cq == cpr - 1 && !last_strip) pk8 &= 0x7fu;  // its lower neighbours are in the next strip
+                }
+                const int cnt = __popc(m);
+                int incl = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
+                int wbase = 0;
+                if (lane == 31) wbase = atomicAdd(&sh.n_sl, incl);
+                wbase = __shfl_sync(0xffffffffu, wbase, 31);
+                int slot = wbase + incl - cnt;
+                uint32_t head = 0;  // offset back to the first bin of the run of on bins (consecutive theta rows) that contains q
+                uint32_t prev = 0xfffffff0u;  // prev + 1 matches no bit position
+                while (m) {
+                    const int q = __ffs(m) - 1;
+                    m &= m - 1;
+                    head = ((uint32_t)q == prev + 1u) ? head + 1u : 0u;
+                    prev = (uint32_t)q;
+                    const uint32_t c = (uint32_t)tile[loc0 + q] & kCountMax;
+                    // strip-list entry: peak (bit 30) | offset back to its run's head (3 bits) | bin index inside the tile (17 bits) | votes (10 bits)
+                    if (slot < sl_lim) slist[slot] = (((pk8 >> q) & 1u) << 30) | (head << 27) | ((loc0 + q) << kCountBits) | c;
+                    ++slot;
                 }
             }
             __syncthreads();
             HOUGH_PT(4);
             const int n_sl = sh.n_sl, on0 = sh.n_on;
-            if (sh.defer || n_sl > P.fSLCAP || on0 + n_sl > P.f_oncap) { give_up = true; break; }  // block-uniform
+            if (n_sl > sl_lim || on0 + n_sl > P.f_oncap) { give_up = true; break; }  // block-uniform
 
             // ---------------- (b) on bins become kOnFlag | on-list index; a bin below another on bin of its chunk joins that
             //                      run's head right away (indices of one chunk are consecutive), the others are singletons
             for (int i = tid; i < n_sl; i += nthr) {
                 const uint32_t ent = slist[i];
-                tile[(ent >> kCountBits) & 0x1ffffu] = (uint16_t)(kOnFlag | (uint32_t)(on0 + i));
-                parent[on0 + i] = (unsigned short)(on0 + i - (int)(ent >> 27));  // bit 27: joins the entry before it
+                const uint32_t loc = (ent >> kCountBits) & 0x1ffffu;
+                const uint16_t en = (uint16_t)(kOnFlag | (uint32_t)(on0 + i));
+                tile[loc] = en;
+                if ((loc & (uint32_t)(S - 1)) == (uint32_t)(S - 1)) ihalo_cur[loc >> (k - 1)] = en;  // last theta row: index halo of the next strip
+                parent[on0 + i] = (unsigned short)(on0 + i - (int)((ent >> 27) & 7u));  // the head of its run inside the chunk
             }
             __syncthreads();
             HOUGH_PT(5);
 
-            // ---------------- (a)+(c) one thread per on bin: local-maximum test and S3 joins, from the same 8 neighbour entries.
-            // A neighbour can beat an on bin only if it is on itself, and then its count is in the strip list (this strip) or in
-            // the count halo (previous strip's last row).
+            // ---------------- (c) one thread per on bin: S3 joins from the entries of its four neighbours of smaller linear index;
+            // the peak flag comes with the strip-list entry.  A neighbour's count, where the deferred row needs it, is in the
+            // strip list (this strip) or in the count halo (previous strip's last row).
             auto ncount = [&](uint32_t en, int tl_nb, int r_nb) -> uint32_t {
                 if (!(en & kOnFlag)) return 0u;
                 return tl_nb >= 0 ? (slist[(int)(en & 0x7fffu) - on0] & kCountMax) : (uint32_t)halo_prev[P.n_rho + r_nb];
             };
-            // The strip list is in scan order, so neighbouring entries belong to the same cluster.  Lane l of a warp takes entry
-            // l * W + (warp-trip index): the 32 lanes of a warp work on 32 far-apart bins and do not fight over one root.
+            // Lane l of a warp takes entry l * W + (warp-trip index): the 32 lanes of a warp work on 32 far-apart bins and do
+            // not fight over one root.  The trips start at the last warp: the first ones have the deferred row to do.
             const int W = (n_sl + 31) >> 5;
-            for (int i0 = tid - lane; i0 < W * 32; i0 += nthr) {
+            for (int i0 = nthr - 32 - (tid - lane); i0 < W * 32; i0 += nthr) {
                 const int i = lane * W + (i0 >> 5);
                 bool pk = false;
                 uint32_t c = 0, L = 0, q0 = 0xffffffffu, q1 = 0xffffffffu, me_idx = 0;
                 if (i < n_sl) {
                     const uint32_t ent = slist[i];
                     c = ent & kCountMax;
-                    const int loc = (int)((ent >> kCountBits) & 0x1ffffu), hoff = (int)(ent >> 27);
+                    pk = (ent >> 30) & 1u;
+                    const int loc = (int)((ent >> kCountBits) & 0x1ffffu), hoff = (int)((ent >> 27) & 7u);
                     const int r = loc >> (k - 1), tl = loc & (S - 1);  // S = 2^(k-1) theta rows per strip
                     const uint32_t me = (uint32_t)(on0 + i);
                     L = (uint32_t)((base + tl) * P.n_rho + r);
                     const uint32_t n0 = fentry_at(P, tile, ihalo_prev, tl, r - 1);
-                    const uint32_t n1 = fentry_at(P, tile, ihalo_prev, tl - 1, r);
+                    const uint32_t n1 = hoff > 0 ? kOnFlag : fentry_at(P, tile, ihalo_prev, tl - 1, r);
                     const uint32_t n2 = fentry_at(P, tile, ihalo_prev, tl - 1, r - 1);
                     const uint32_t n3 = fentry_at(P, tile, ihalo_prev, tl - 1, r + 1);
-                    // joins with the neighbours of smaller linear index; a join is skipped when other joins already imply it.
-                    // At most two partners remain; they go through ONE union call site so that the lanes of a warp stay together.
+                    // a join is skipped when other joins already imply it.  At most two partners remain; they go through ONE
+                    // union call site so that the lanes of a warp stay together.
                     constexpr uint32_t kNone = 0xffffffffu;
-                    if (hoff > 0 || (n1 & kOnFlag)) {
+                    if (n1 & kOnFlag) {
                         if (hoff == 0) q0 = n1 & 0x7fffu;
                         if ((n0 & kOnFlag) && !(n2 & kOnFlag)) q1 = n0 & 0x7fffu;
                     } else {
@@ -417,17 +484,6 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     }
                     if (q0 == kNone) { q0 = q1; q1 = kNone; }
                     me_idx = me;
-                    if (tl < S - 1 || last_strip) {
-                        const bool below = tl + 1 < S && base + tl + 1 < P.n_theta;  // else: beyond the grid (last strip)
-                        const uint32_t n4 = fentry_at(P, tile, ihalo_prev, tl, r + 1);
-                        const uint32_t n5 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r - 1) : 0u;
-                        const uint32_t n6 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r) : 0u;
-                        const uint32_t n7 = below ? fentry_at(P, tile, ihalo_prev, tl + 1, r + 1) : 0u;
-                        // no short-circuit: straight-line predicated code instead of eight divergent exits
-                        pk = (ncount(n2, tl - 1, r - 1) < c) & (ncount(n1, tl - 1, r) < c) & (ncount(n3, tl - 1, r + 1) < c) &
-                             (ncount(n0, tl, r - 1) < c) & (ncount(n4, tl, r + 1) <= c) & (ncount(n5, tl + 1, r - 1) <= c) &
-                             (ncount(n6, tl + 1, r) <= c) & (ncount(n7, tl + 1, r + 1) <= c);
-                    }
                 }
 #pragma unroll 1
                 for (int kk = 0; kk < 2; ++kk) {
@@ -472,13 +528,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 }
             }
             HOUGH_PT(9);
-            if (!last_strip) {  // entries of the last theta row, for the next strip's joins and deferred-row peaks
-                for (int r = tid; r < P.n_rho; r += nthr) {
-                    const uint16_t en = tile[r * S + S - 1];
-                    ihalo_cur[r] = (en & kOnFlag) ? en : (uint16_t)0;
-                }
-            }
-            if (tid == 0) { sh.n_on = on0 + n_sl; sh.n_sl = 0; }
+            if (tid == 0) { sh.n_on = on0 + n_sl; sh.n_sl = 0; sh.n_ch = 0; }
             __syncthreads();  // the tile may be zeroed again
             HOUGH_PT(6);
         }  // strips
