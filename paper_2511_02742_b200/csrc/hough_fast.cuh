@@ -320,13 +320,17 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             // (chunk index | on mask << 16) to a list that grows down from the end of the strip list: one ballot, one atomic
             // per warp trip.  Pass 2 (dense: one thread per on chunk) expands them into the strip list's per-bin entries.
             {
-                const uint4* t4 = reinterpret_cast<const uint4*>(tile);
+                // nthr is a multiple of cpr, so a thread stays in one chunk column: its shared-memory address and its halo slot
+                // advance by constants, and only the threads of the last chunk column save the count halo
                 const int i_lo = r_lo * cpr, i_hi = (r_hi + 1) * cpr;  // only rho rows some hit can reach
-                for (int i0 = i_lo + tid - lane; i0 < i_hi; i0 += nthr) {
-                    const int idx = i0 + lane;
+                const bool halo_lane = (tid & (cpr - 1)) == cpr - 1;
+                uint16_t* hp = halo_cur + r_lo + tid / cpr;
+                const uint32_t a_end = tile_base + 16u * (uint32_t)i_hi;
+                for (uint32_t a = tile_base + 16u * (uint32_t)(i_lo + tid); a - 16u * lane < a_end; a += 16u * nthr, hp += nthr / cpr) {
                     uint32_t m = 0;  // bit q set <=> count q of this chunk is on
-                    if (idx < i_hi) {
-                        const uint4 w = t4[idx];
+                    if (a < a_end) {
+                        uint4 w;
+                        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(a));
                         // counts are below 2^15 (at most one vote per hit, fHB <= 32767), so adding 2^15 - T to both
                         // halfwords sets their top bits exactly where count >= T, without a carry between them
                         const uint32_t gx = (w.x + tadd) & 0x80008000u, gy = (w.y + tadd) & 0x80008000u;
@@ -338,10 +342,9 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                             if (((w.x + oadd) | (w.y + oadd) | (w.z + oadd) | (w.w + oadd)) & 0x80008000u) sh.defer = 1;
                         }
                         // theta rows beyond n_theta hold no votes (checked_vote masks them), so m needs no masking
-                        if ((idx & (cpr - 1)) == cpr - 1) {  // last chunk of a rho row: its two last counts are the next strip's halo
-                            const int r = idx / cpr;         // (rows no vote can reach are never scanned: they stay 0 from the event's start)
-                            halo_cur[r] = (uint16_t)(w.w & 0xffffu);
-                            halo_cur[P.n_rho + r] = (uint16_t)(w.w >> 16);
+                        if (halo_lane) {  // the row's two last counts are the next strip's count halo
+                            hp[0] = (uint16_t)(w.w & 0xffffu);  // (rows no vote can reach are never scanned: they stay 0 from the event's start)
+                            hp[P.n_rho] = (uint16_t)(w.w >> 16);
                         }
                     }
                     const unsigned bal = __ballot_sync(0xffffffffu, m != 0);
@@ -349,7 +352,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     int cb = 0;
                     if (lane == 0) cb = atomicAdd(&sh.n_ch, __popc(bal));
                     cb = __shfl_sync(0xffffffffu, cb, 0) + __popc(bal & lanemask_lt());
-                    if (m != 0 && cb < P.fSLCAP) slist[P.fSLCAP - 1 - cb] = (uint32_t)idx | (m << 16);
+                    if (m != 0 && cb < P.fSLCAP) slist[P.fSLCAP - 1 - cb] = ((a - tile_base) >> 4) | (m << 16);
                 }
             }
             __syncthreads();

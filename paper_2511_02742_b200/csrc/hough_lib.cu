@@ -346,7 +346,8 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
             if ((long long)d->n_rho * rows >= (1ll << 17)) continue;  // strip-list entries hold a 17-bit tile index
             int hb = (int)align_up((size_t)(d->max_hits_per_event < 32 ? 32 : d->max_hits_per_event), 32);
             if (hb > 8192) hb = 8192;
-            int slcap = env_int("HOUGH_FAST_SLCAP", 2048 * c.G > 8192 ? 8192 : 2048 * c.G), pcap = env_int("HOUGH_FAST_PCAP", 4096);
+            // the strip list also holds the strip's on-chunk list at its end (hough_fast.cuh S2)
+            int slcap = env_int("HOUGH_FAST_SLCAP", 2560 * c.G > 10240 ? 10240 : 2560 * c.G), pcap = env_int("HOUGH_FAST_PCAP", 3584);
             int oncap = env_int("HOUGH_FAST_ONCAP", 12288);
             if (oncap > 32767) oncap = 32767;
             if (oncap * 4 > tile) oncap = tile / 4;  // root tags reuse the tile
