@@ -124,16 +124,19 @@ __device__ __forceinline__ void fast_vote(const int2* __restrict__ hits, int n, 
     const int4* p = reinterpret_cast<const int4*>(hits) + warp;
     int i = warp;
 #pragma unroll 1
-    for (; i + 3 * NW < npairs; i += 4 * NW, p += 4 * NW) {
-        const int4 h0 = p[0], h1 = p[NW], h2 = p[2 * NW], h3 = p[3 * NW];
-        HOUGH_VOTE1(h0.x, h0.y)
-        HOUGH_VOTE1(h0.z, h0.w)
-        HOUGH_VOTE1(h1.x, h1.y)
-        HOUGH_VOTE1(h1.z, h1.w)
-        HOUGH_VOTE1(h2.x, h2.y)
-        HOUGH_VOTE1(h2.z, h2.w)
-        HOUGH_VOTE1(h3.x, h3.y)
-        HOUGH_VOTE1(h3.z, h3.w)
+    for (; i + 7 * NW < npairs; i += 8 * NW, p += 8 * NW) {
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            const int4 h0 = p[(4 * hh) * NW], h1 = p[(4 * hh + 1) * NW], h2 = p[(4 * hh + 2) * NW], h3 = p[(4 * hh + 3) * NW];
+            HOUGH_VOTE1(h0.x, h0.y)
+            HOUGH_VOTE1(h0.z, h0.w)
+            HOUGH_VOTE1(h1.x, h1.y)
+            HOUGH_VOTE1(h1.z, h1.w)
+            HOUGH_VOTE1(h2.x, h2.y)
+            HOUGH_VOTE1(h2.z, h2.w)
+            HOUGH_VOTE1(h3.x, h3.y)
+            HOUGH_VOTE1(h3.z, h3.w)
+        }
     }
 #pragma unroll 1
     for (; i < npairs; i += NW, p += NW) {
