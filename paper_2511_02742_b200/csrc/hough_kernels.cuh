@@ -596,20 +596,40 @@ hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float*
             trip[s] = make_int4(__ldg(P.Cq + t), __ldg(P.Sq + t), P.Oq - (r << P.F) - half, 0);
         }
         __syncthreads();
-        for (long long i = g0 + tid; i < g1; i += nthr) {
-            const float uf = __ldg(u + i), vf = __ldg(v + i);
-            int label = -1;
-            if ((fabsf(uf) <= P.coord_max) && (fabsf(vf) <= P.coord_max)) {
-                const int uq = __float2int_rn(uf * P.hit_scale), vq = __float2int_rn(vf * P.hit_scale);
-                unsigned best = 0xffffffffu;
-                for (int s = 0; s < nk; ++s) {
-                    const int4 c = trip[s];
-                    const int ev = uq * c.x + (vq * c.y + c.z);
+        // HPT hits per thread and trip: one broadcast load of a candidate triple serves HPT residuals.  best starts at
+        // W_q + 1, so "|e| < best" alone is the eligibility test and the strict compare keeps the lowest slot on ties.
+        constexpr int HPT = 4;
+        const unsigned best0 = (unsigned)P.Wq + 1u;
+        for (long long i0 = g0 + tid; i0 < g1; i0 += (long long)HPT * nthr) {
+            int uq[HPT], vq[HPT], label[HPT];
+            unsigned best[HPT];
+            bool ok[HPT];
+#pragma unroll
+            for (int j = 0; j < HPT; ++j) {
+                const long long i = i0 + (long long)j * nthr;
+                float uf = 0.f, vf = 0.f;
+                if (i < g1) { uf = __ldg(u + i); vf = __ldg(v + i); }
+                ok[j] = (fabsf(uf) <= P.coord_max) && (fabsf(vf) <= P.coord_max);  // false for NaN
+                uq[j] = ok[j] ? __float2int_rn(uf * P.hit_scale) : 0;
+                vq[j] = ok[j] ? __float2int_rn(vf * P.hit_scale) : 0;
+                best[j] = best0;
+                label[j] = -1;
+            }
+#pragma unroll 2
+            for (int s = 0; s < nk; ++s) {
+                const int4 c = trip[s];
+#pragma unroll
+                for (int j = 0; j < HPT; ++j) {
+                    const int ev = uq[j] * c.x + (vq[j] * c.y + c.z);
                     const unsigned ae = (unsigned)abs(ev);
-                    if (ae <= (unsigned)P.Wq && ae < best) { best = ae; label = s; }
+                    if (ae < best[j]) { best[j] = ae; label[j] = s; }
                 }
             }
-            labels[i] = label;
+#pragma unroll
+            for (int j = 0; j < HPT; ++j) {
+                const long long i = i0 + (long long)j * nthr;
+                if (i < g1) labels[i] = ok[j] ? label[j] : -1;
+            }
         }
     }
 }
