@@ -355,7 +355,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one hough_event_kernel launch, from the ncu --set full capture under
 # profiles/ (workload name -> bytes); None until a capture of that workload exists.
-TRAFFIC_BYTES_PER_LAUNCH = {"cfg3_100k_events_pileup40": 2643605104}   # profiles/r1_fast_kernel_ncu.md
+TRAFFIC_BYTES_PER_LAUNCH = {"cfg3_100k_events_pileup40": 2637558016}   # dram read + write of one launch, profiles/r1_fast_kernel_ncu.md
 
 
 def main():
