@@ -2,8 +2,8 @@
 //
 // Same results as hough_event_kernel (hough_kernels.cuh), for the common case only; an event that does not fit the
 // fast path's capacities is appended to a "deferred" list and processed afterwards by the general kernel:
-//     more hits than the staged-hit buffer, a bin count above 1023, more on bins in one strip than the strip list
-//     holds, more on bins / peaks in the event than the parent / peak arrays hold, more ties at the K-th vote count
+//     more hits than the staged-hit buffer, a bin count above 1023, more on bins + on chunks in one strip than the
+//     strip list holds, more on bins / peaks in the event than the parent / peak arrays hold, more ties at the K-th vote count
 //     than the tie buffer.
 //
 // Per event (one CTA at a time):
@@ -12,8 +12,11 @@
 //   S1  vote      lane <-> 32-bit word column (2 theta rows), 2 IMAD + SHF + LOP3 + RED per vote:
 //                 the tile base is folded into the fixed-point offset, so ((a >> (F - k)) & ~(2^k - 1)) | column
 //                 IS the shared-memory address of the counter word                                   (Eq. 4.1)
-//   S2  scan      16-byte chunks -> compact list of the strip's on bins -> one thread per on bin:
-//                 (a) strict-local-maximum test on the counts (1 theta row of halo kept between strips) (L94, L106)
+//   S2  scan      pass 1 (sparse): 16-byte chunks (8 counts) -> list of the strip's on chunks, one ballot + one atomic per
+//                 warp trip; the strip's last two theta rows are saved as the next strip's count halo on the way
+//                 pass 2 (dense): one thread per on chunk: (a) strict-local-maximum test of its 8 bins at once on packed
+//                 halfwords, straight from the counts (1 theta row of halo kept between strips)        (L94, L106)
+//                 -> per-bin strip-list entries (peak flag | offset to the run's head | tile index | votes)
 //                 (b) the on bin's tile entry is overwritten with 0x8000 | its index in the event's on list
 //   S3  clusters  (c) each on bin reads the entries of its four earlier neighbours straight from the tile and joins
 //                 them in a union-find over on-list indices (16-bit parents in shared memory)         (keyword L29)

@@ -1,0 +1,128 @@
+"""CPU checks of the integer identities the fast kernel's design rests on (hough_fast.cuh), modelled in numpy with the
+kernel's word widths and compared with the oracle's definitions.  They do not run the kernel (the `-m gpu` parity tests
+do); they pin the derivations stated in DESIGN.md section 7.1 at sizes the GPU tests cannot enumerate:
+
+  * address folding: ((a' >> (F - k)) & ~(2^k - 1)) | column is the shared-memory address of the counter word,
+    a' = u_q C + v_q S + O_q + (tile_base << (F - k)) in wrapping 32-bit arithmetic;
+  * the threshold test on packed halfwords, (w + (2^15 - T) * 0x00010001) & 0x80008000;
+  * the strict-local-maximum test of the 8 bins of a chunk on packed halfwords (column maxima, halfword shifts by byte
+    permutation, borrow-free compares) == oracle O4 (`hough_def.peaks`).
+"""
+import numpy as np
+import pytest
+
+from oracle import hough_def as D
+from util import std_params
+
+U32 = np.uint64(0xFFFFFFFF)
+
+
+def _u32(x):
+    return np.asarray(x, dtype=np.uint64) & U32
+
+
+@pytest.mark.parametrize("n_theta,n_rho,G", [(512, 512, 2), (256, 256, 2), (256, 512, 1), (180, 256, 2), (128, 128, 1), (1024, 1024, 1)])
+def test_vote_address_folding(n_theta, n_rho, G):
+    """For every in-range (hit, theta) the folded 32-bit expression is tile_base + r * row_bytes + column, r = a >> F."""
+    p = std_params(n_theta, n_rho)
+    k = D.constants(p)
+    row_bytes = 128 * G
+    kk = int(np.log2(row_bytes))
+    sh = k.F - kk
+    assert sh >= 0
+    tile_base = 1024  # dynamic shared memory window offset: a multiple of the row size, below 4096
+    assert ((4096 << sh) + (n_rho << k.F)) <= 0xFFFFFFFF  # the plan's admission test for the fast path
+    rng = np.random.default_rng(7)
+    lim = int(p.coord_max * (1 << k.H))
+    uq = rng.integers(-lim, lim + 1, 4000)
+    vq = rng.integers(-lim, lim + 1, 4000)
+    C = np.asarray(k.Cq, dtype=np.int64)
+    S = np.asarray(k.Sq, dtype=np.int64)
+    a = uq[:, None] * C[None, :] + vq[:, None] * S[None, :] + k.Oq  # exact
+    r = a >> k.F
+    inr = (r >= 0) & (r < n_rho)
+    assert inr.any()
+    Oq2 = (k.Oq + (tile_base << sh)) & 0xFFFFFFFF
+    a32 = _u32(_u32(uq[:, None] * C[None, :]) + _u32(_u32(vq[:, None] * S[None, :]) + np.uint64(Oq2)))  # wrapping IMADs
+    amask = np.uint64((~((1 << kk) - 1)) & 0xFFFFFFFF)
+    col = np.uint64(4 * 13)  # any lane's column offset inside the row (< row_bytes, word aligned)
+    addr = ((a32 >> np.uint64(sh)) & amask) | col
+    want = tile_base + r * row_bytes + int(col)
+    np.testing.assert_array_equal(addr[inr].astype(np.int64), want[inr])
+
+
+@pytest.mark.parametrize("T", [1, 19, 20, 24, 1023])
+def test_packed_threshold_test(T):
+    rng = np.random.default_rng(T)
+    lo = rng.integers(0, 1 << 15, 20000, dtype=np.uint64)
+    hi = rng.integers(0, 1 << 15, 20000, dtype=np.uint64)
+    for near in (T - 1, T, T + 1):  # make sure the boundary is hit
+        lo[rng.integers(0, lo.size, 500)] = max(near, 0)
+        hi[rng.integers(0, hi.size, 500)] = max(near, 0)
+    w = lo | (hi << np.uint64(16))
+    tadd = np.uint64(((0x8000 - T) * 0x00010001) & 0xFFFFFFFF)
+    g = _u32(w + tadd) & np.uint64(0x80008000)
+    np.testing.assert_array_equal((g & np.uint64(0x8000)) != 0, lo >= T)
+    np.testing.assert_array_equal((g & np.uint64(0x80000000)) != 0, hi >= T)
+
+
+def _vmaxu2(a, b):
+    lo = np.maximum(a & np.uint64(0xFFFF), b & np.uint64(0xFFFF))
+    hi = np.maximum(a >> np.uint64(16), b >> np.uint64(16))
+    return lo | (hi << np.uint64(16))
+
+
+def _perm5432(x, y):
+    """__byte_perm(x, y, 0x5432): low half = high half of x, high half = low half of y."""
+    return (x >> np.uint64(16)) | ((y & np.uint64(0xFFFF)) << np.uint64(16))
+
+
+def _pack(c8):
+    """8 counts (theta fastest) -> 4 words, word j = (count 2j, count 2j + 1)."""
+    c8 = np.asarray(c8, dtype=np.uint64)
+    return [c8[2 * j] | (c8[2 * j + 1] << np.uint64(16)) for j in range(4)]
+
+
+def _chunk_peak_mask(a8, b8, c8, am, bm, cm, ap, bp, cp, T):
+    """The kernel's pass-2 arithmetic for one chunk: rows r-1 / r / r+1 (a / b / c), *m = theta row before the chunk,
+    *p = theta row after it.  Returns the 8-bit peak mask."""
+    A, B, C = _pack(a8), _pack(b8), _pack(c8)
+    em = np.uint64(max(am, bm, cm))
+    ep = np.uint64(max(ap, bp, cp))
+    V = [_vmaxu2(_vmaxu2(A[j], B[j]), C[j]) for j in range(4)]
+    Vm = [_perm5432(_u32(em << np.uint64(16)), V[0]), _perm5432(V[0], V[1]), _perm5432(V[1], V[2]), _perm5432(V[2], V[3]),
+          _perm5432(V[3], ep)]
+    mask = 0
+    for j in range(4):
+        bh = B[j] | np.uint64(0x80008000)
+        sm = _vmaxu2(Vm[j], A[j])
+        nm = _vmaxu2(Vm[j + 1], C[j])
+        g = _u32(bh - sm - np.uint64(0x00010001)) & _u32(bh - nm) & np.uint64(0x80008000)
+        bits = int(((g >> np.uint64(15)) | (g >> np.uint64(30))) & np.uint64(3))
+        mask |= bits << (2 * j)
+    on = sum(1 << q for q in range(8) if b8[q] >= T)
+    return mask & on
+
+
+@pytest.mark.parametrize("seed,hi", [(0, 4), (1, 40), (2, 1000), (3, 32767)])
+def test_packed_local_maximum_test_equals_oracle_peaks(seed, hi):
+    """Random small accumulators with many ties; every 8-theta chunk (all positions, borders included) against O4."""
+    rng = np.random.default_rng(seed)
+    n_theta, n_rho, T = 24, 9, 2
+    p = std_params(n_theta, n_rho, T=T)
+    for _ in range(12):
+        acc = rng.integers(0, hi + 1, (n_theta, n_rho)).astype(np.int64)
+        want = set(D.peaks(acc, p))
+
+        def at(t, r):
+            return int(acc[t, r]) if 0 <= t < n_theta and 0 <= r < n_rho else 0
+
+        got = set()
+        for r in range(n_rho):
+            for t0 in range(0, n_theta, 8):
+                m = _chunk_peak_mask([at(t0 + q, r - 1) for q in range(8)], [at(t0 + q, r) for q in range(8)],
+                                     [at(t0 + q, r + 1) for q in range(8)],
+                                     at(t0 - 1, r - 1), at(t0 - 1, r), at(t0 - 1, r + 1),
+                                     at(t0 + 8, r - 1), at(t0 + 8, r), at(t0 + 8, r + 1), T)
+                got |= {(t0 + q, r) for q in range(8) if (m >> q) & 1}
+        assert got == want
