@@ -497,9 +497,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 #pragma unroll 1
                 for (int kk = 0; kk < 2; ++kk) {
                     const uint32_t q = kk ? q1 : q0;
-#if !defined(HOUGH_EXP) || HOUGH_EXP != 1
                     if (q != 0xffffffffu) suf_union(parent, me_idx, q);
-#endif
                     if (__ballot_sync(0xffffffffu, q1 != 0xffffffffu) == 0) break;  // warp-uniform
                 }
                 __syncwarp();  // reconverge after the data-dependent union loops
