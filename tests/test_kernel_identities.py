@@ -6,7 +6,9 @@ do); they pin the derivations stated in DESIGN.md section 7.1 at sizes the GPU t
     a' = u_q C + v_q S + O_q + (tile_base << (F - k)) in wrapping 32-bit arithmetic;
   * the threshold test on packed halfwords, (w + (2^15 - T) * 0x00010001) & 0x80008000;
   * the strict-local-maximum test of the 8 bins of a chunk on packed halfwords (column maxima, halfword shifts by byte
-    permutation, borrow-free compares) == oracle O4 (`hough_def.peaks`).
+    permutation, borrow-free compares) == oracle O4 (`hough_def.peaks`);
+  * the S3 join rules (prelinks inside a chunk, at most two explicit joins per on bin, implied joins skipped) connect
+    exactly the 8-connected components (`scipy.ndimage.label`).
 """
 import numpy as np
 import pytest
@@ -126,3 +128,69 @@ def test_packed_local_maximum_test_equals_oracle_peaks(seed, hi):
                                      at(t0 + 8, r - 1), at(t0 + 8, r), at(t0 + 8, r + 1), T)
                 got |= {(t0 + q, r) for q in range(8) if (m >> q) & 1}
         assert got == want
+
+
+def _join_edges(mask, chunk=8):
+    """The fast kernel's S3 join rules (hough_fast.cuh, step (c)) on a whole on mask [n_theta][n_rho]: prelinks inside a
+    chunk of `chunk` consecutive theta rows, then per on bin at most two explicit joins with neighbours of smaller
+    linear index; joins that other joins imply are skipped.  Returns the list of joined pairs."""
+    n_theta, n_rho = mask.shape
+
+    def on(t, r):
+        return 0 <= t < n_theta and 0 <= r < n_rho and bool(mask[t, r])
+
+    edges = []
+    for t in range(n_theta):
+        for r in range(n_rho):
+            if not mask[t, r]:
+                continue
+            me = (t, r)
+            hoff = on(t - 1, r) and (t % chunk) != 0  # the bin above is on and in the same chunk: prelinked to its run
+            if hoff:
+                edges.append((me, (t - 1, r)))        # (through the run's head; same component)
+            n0, n1, n2, n3 = on(t, r - 1), on(t - 1, r), on(t - 1, r - 1), on(t - 1, r + 1)
+            if n1:
+                if not hoff:
+                    edges.append((me, (t - 1, r)))
+                if n0 and not n2:
+                    edges.append((me, (t, r - 1)))
+            else:
+                if n0:
+                    edges.append((me, (t, r - 1)))
+                elif n2:
+                    edges.append((me, (t - 1, r - 1)))
+                if n3:
+                    edges.append((me, (t - 1, r + 1)))
+    return edges
+
+
+@pytest.mark.parametrize("seed,density", [(0, 0.2), (1, 0.35), (2, 0.5), (3, 0.65), (4, 0.9)])
+def test_join_rules_give_the_8_connected_components(seed, density):
+    """The pruned joins connect exactly the 8-connected components (scipy.ndimage.label with the 3 x 3 structure), on
+    random masks of every density, with chunk seams every 8 theta rows."""
+    ndimage = pytest.importorskip("scipy.ndimage")
+    rng = np.random.default_rng(seed)
+    for _ in range(6):
+        mask = rng.random((27, 19)) < density
+        parent = {}
+
+        def find(x):
+            while parent.setdefault(x, x) != x:
+                parent[x] = parent[parent[x]]
+                x = parent[x]
+            return x
+
+        n_explicit = {}
+        for a, b in _join_edges(mask):
+            assert mask[a] and mask[b]
+            assert max(abs(a[0] - b[0]), abs(a[1] - b[1])) == 1  # only 8-neighbours are ever joined
+            n_explicit[a] = n_explicit.get(a, 0) + 1
+            ra, rb = find(a), find(b)
+            if ra != rb:
+                parent[max(ra, rb)] = min(ra, rb)
+        assert all(v <= 3 for v in n_explicit.values())  # one prelink + at most two explicit partners
+        lab, n = ndimage.label(mask, structure=np.ones((3, 3), dtype=int))
+        roots = {}
+        for t, r in zip(*np.nonzero(mask)):
+            roots.setdefault(find((int(t), int(r))), set()).add(int(lab[t, r]))
+        assert len(roots) == n and all(len(s) == 1 for s in roots.values())
