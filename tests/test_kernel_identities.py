@@ -8,7 +8,8 @@ do); they pin the derivations stated in DESIGN.md section 7.1 at sizes the GPU t
   * the strict-local-maximum test of the 8 bins of a chunk on packed halfwords (column maxima, halfword shifts by byte
     permutation, borrow-free compares) == oracle O4 (`hough_def.peaks`);
   * the S3 join rules (prelinks inside a chunk, at most two explicit joins per on bin, implied joins skipped) connect
-    exactly the 8-connected components (`scipy.ndimage.label`).
+    exactly the 8-connected components (`scipy.ndimage.label`);
+  * the Cauchy-Schwarz bounds behind the unchecked vote loop (safe radius) and the restricted clear / scan (reachable rows).
 """
 import numpy as np
 import pytest
@@ -194,3 +195,51 @@ def test_join_rules_give_the_8_connected_components(seed, density):
         for t, r in zip(*np.nonzero(mask)):
             roots.setdefault(find((int(t), int(r))), set()).add(int(lab[t, r]))
         assert len(roots) == n and all(len(s) == 1 for s in roots.values())
+
+
+def _grid_cases():
+    out = [std_params(nt, nr) for nt, nr in [(180, 256), (256, 256), (256, 512), (512, 512), (128, 128), (1024, 1024)]]
+    out.append(D.Params(n_theta=180, n_rho=1000, rho_min=-500.0, rho_max=500.0, coord_max=256.0, vote_threshold=24,
+                        assign_window=1.0, max_candidates=128))  # the paper's CPU grid
+    return out
+
+
+@pytest.mark.parametrize("p", _grid_cases(), ids=lambda p: f"{p.n_theta}x{p.n_rho}")
+def test_safe_radius_and_reachable_rows_bounds(p):
+    """Two Cauchy-Schwarz bounds the kernels rely on (hough_lib.cu: r2safe, Mq1; hough_fast.cuh: r_lo, r_hi), checked
+    against the exact integer a(h, t) of the definition:
+      * u_q^2 + v_q^2 <= r2safe  =>  0 <= a < n_rho 2^F for EVERY theta (such hits vote without a range test);
+      * every vote of an event falls into rho rows [(O_q - B) >> F, (O_q + B) >> F], B = (ceil(M) + 1)(ceil(sqrt(r2max)) + 1)."""
+    import math
+    k = D.constants(p)
+    C = np.asarray(k.Cq, dtype=np.int64)
+    S = np.asarray(k.Sq, dtype=np.int64)
+    top = p.n_rho * (1 << k.F)
+    m = min(float(k.Oq), float(top) - 1.0 - float(k.Oq))
+    assert m > 0
+    R = m / (k.M + 1.0)
+    r2safe = int(math.floor(R * R * (1.0 - 1e-9)) - 1.0)
+    lim = int(p.coord_max * (1 << k.H))
+    rng = np.random.default_rng(11)
+    # hits on and just inside the safe circle, at many angles (the extreme a is reached near theta = the hit's own angle)
+    ang = np.concatenate([rng.random(3000) * 2 * np.pi, np.linspace(0, 2 * np.pi, 721)])
+    rad = math.sqrt(r2safe)
+    uq = np.clip(np.trunc(rad * np.cos(ang)).astype(np.int64), -lim, lim)
+    vq = np.clip(np.trunc(rad * np.sin(ang)).astype(np.int64), -lim, lim)
+    keep = uq * uq + vq * vq <= r2safe
+    uq, vq = uq[keep], vq[keep]
+    assert uq.size > 1000
+    a = uq[:, None] * C[None, :] + vq[:, None] * S[None, :] + k.Oq
+    assert a.min() >= 0 and a.max() < top
+    # reachable rows of a random event (any valid hits)
+    Mq1 = int(math.ceil(k.M)) + 1
+    for n in (1, 7, 300):
+        eu = rng.integers(-lim, lim + 1, n)
+        ev = rng.integers(-lim, lim + 1, n)
+        r2max = int((eu * eu + ev * ev).max())
+        B = Mq1 * (int(math.ceil(math.sqrt(float(r2max)))) + 1)
+        r_lo = max((k.Oq - B) >> k.F, 0)
+        r_hi = min((k.Oq + B) >> k.F, p.n_rho - 1)
+        rows = (eu[:, None] * C[None, :] + ev[:, None] * S[None, :] + k.Oq) >> k.F
+        inr = (rows >= 0) & (rows < p.n_rho)
+        assert rows[inr].min() >= r_lo and rows[inr].max() <= r_hi
