@@ -273,6 +273,7 @@ def run_ours(args):
     ms_step = ms_total / args.steps
     ms_find = statistics.mean(e[0].elapsed_time(e[1]) for e in evs)
     ms_assign = statistics.mean(e[1].elapsed_time(e[2]) for e in evs)
+    step_ms = [e[0].elapsed_time(e[2]) for e in evs]
     events_all = sum_over_ranks(float(n_events))
     hits_all = sum_over_ranks(float(n_hits))
     value = events_all / (ms_step * 1e-3)
@@ -344,6 +345,7 @@ def run_ours(args):
                 "config": config_of(wl, n_events, n_hits, {"parallelism": f"events sharded over {world} GPU(s), no collective",
                                                            "plan": info, "status_word": status, "gen_s": round(t_gen, 1)}),
                 "kernel_ms": {"hough_find_clusters": ms_find, "hough_assign_hits": ms_assign},
+                "ms_per_step_median": statistics.median(step_ms), "ms_per_step_best": min(step_ms),     # this rank's steps
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
     H.hough_plan_destroy(plan)
     if dist is not None:
