@@ -104,6 +104,41 @@ def test_p1_frac_bits_of_all_config_grids(impl):
         assert F == F_exp and Oq == 2 ** 29 and Cq[0] == 32768 and Sq[32] == 32768
 
 
+# ----------------------------------------------------------------------------- P1b rounding rules (reading A5)
+def _quantised(impl, x):
+    """u_q and v_q of the hit (x, -x) as the oracle computes them, read off the two axis rows of a grid with d_rho = 2^-H:
+    there C_q[0] = S_q[1] = 2^F exactly, so r = q + n_rho / 2 in both rows."""
+    p = D.Params(2, 32, -16 / 64, 16 / 64, 0.2, 1, 1 / 64, 4, 6, -1)
+    acc = np.asarray(impl.vote(np.array([x], np.float32), np.array([-x], np.float32), p))
+    assert acc[0].sum() == 1 and acc[1].sum() == 1
+    return int(np.argmax(acc[0])) - 16, int(np.argmax(acc[1])) - 16
+
+
+def test_p1b_hit_rounding_is_ties_to_even(impl):
+    rows = [r for r in read_golden_table("tie_rounding.txt") if r[0] == "hit"]
+    assert len(rows) == 7
+    for _, x, q in rows:
+        x, q = float(x), int(q)
+        assert float(np.float32(x)) == x and (x * 128) % 2 == 1            # an exact tie in fp32
+        uq, vq = _quantised(impl, x)
+        assert uq == q, (x, uq, q)
+        assert vq == -q, (x, vq, q)                                          # rint is odd-symmetric
+    # non-ties still round to nearest
+    assert _quantised(impl, 0.0234375 + 2 ** -12)[0] == 2 and _quantised(impl, 0.0390625 + 2 ** -12)[0] == 3
+
+
+def test_p1b_offset_and_window_round_half_away(impl):
+    rows = [r for r in read_golden_table("tie_rounding.txt") if r[0] == "const"]
+    assert len(rows) == 2
+    for _, rho_min, w, oq, wq in rows:
+        rho_min, w = float(rho_min), float(w)
+        p = D.Params(8, 64, rho_min, rho_min + 64.0, 20.0, 3, w, 4, 6, 8)
+        assert (p.rho_max - p.rho_min) / p.n_rho == 1.0
+        H, F, Oq, Wq, _, _ = impl.constants(p)
+        assert (H, F) == (6, 8)
+        assert Oq == int(oq) and Wq == int(wq)
+
+
 # ----------------------------------------------------------------------------- P2 table CRC
 def test_p2_table_crc32(impl):
     for n_theta, crc in read_golden_table("table_crc32.txt"):
@@ -505,6 +540,19 @@ def edge_cases():
     # non-power-of-two d_rho and odd n_theta
     pn = D.Params(45, 77, -230.0, 245.0, 250.0, 6, 3.0, 16)
     cases.append(("odd_grid_nonpow2_drho", pn, uu, vv))
+    # rounding ties (reading A5; goldens in tests/golden/tie_rounding.txt): hit coordinates at odd multiples of 2^-(H+1) on a
+    # grid whose axis rows resolve single fixed-point steps, and offset / window constants with a fractional part of 1/2
+    ties = np.array([0.0078125, 0.0234375, 0.0390625, 0.0546875, -0.0078125, -0.0234375, -0.0390625, 0.0234375, 0.0390625], f32)
+    cases.append(("hit_rounding_ties", D.Params(2, 32, -16 / 64, 16 / 64, 0.2, 1, 1 / 64, 16, 6, -1), ties, -ties))
+    for nm, rmin, w in (("llround_ties_pos_offset", -100.001953125, 1.001953125), ("llround_ties_neg_offset", 100.001953125, 2.501953125)):
+        pc = D.Params(8, 64, rmin, rmin + 64.0, 20.0, 3, w, 4, 6, 8)
+        sgn = -1.0 if rmin > 0 else 1.0
+        cases.append((nm, pc, (sgn * np.linspace(-18, 18, 40)).astype(f32), np.linspace(-15, 19, 40).astype(f32)))
+    # coordinates beyond 2^15 fixed-point units (coord_max 1000, H = 6): u_q^2 + v_q^2 exceeds 32 bits at the corners
+    pw = D.Params(64, 512, -1415.0, 1415.0, 1000.0, 3, 6.0, 16, 6, -1)
+    cw_u = np.concatenate([np.full(6, 1000.0, f32), np.full(6, -1000.0, f32), np.linspace(-990, 990, 12).astype(f32)])
+    cw_v = np.concatenate([np.linspace(985, 1000, 6).astype(f32), np.linspace(-1000, -985, 6).astype(f32), np.linspace(-30, 30, 12).astype(f32)])
+    cases.append(("wide_coordinates_corner_hits", pw, cw_u, cw_v))
     return cases
 
 
