@@ -48,7 +48,13 @@ typedef enum {
 } hough_status;
 
 enum { HOUGH_I32 = 0, HOUGH_U16 = 1 };            /* count_dtype: element type of accumulators dumped by hough_vote */
-enum { HOUGH_STATUS_EVENT_TOO_LONG = 1, HOUGH_STATUS_BAD_OFFSETS = 2 };   /* bits of the device status word */
+enum { HOUGH_STATUS_EVENT_TOO_LONG = 1, HOUGH_STATUS_BAD_OFFSETS = 2,      /* bits of the device status word */
+       HOUGH_STATUS_INTERNAL = 4 };   /* set only by the -DHOUGH_BOUNDS debug build: an index check inside a kernel failed */
+/* hough_plan_desc_t.flags.  Both change only WHICH kernel computes an event, never a result:
+ *   HOUGH_FLAG_GENERAL_ONLY  every event goes through the general kernel (the shared-memory-only fast kernel is not used)
+ *   HOUGH_FLAG_SMALL_LISTS   the fast kernel's per-event lists get their smallest capacities, so that ordinary events
+ *                            overflow them and are handed to the general kernel (exercises that hand-over in tests) */
+enum { HOUGH_FLAG_GENERAL_ONLY = 1, HOUGH_FLAG_SMALL_LISTS = 2 };
 
 typedef struct hough_plan hough_plan_t;           /* opaque; created and destroyed by the library */
 
@@ -70,7 +76,7 @@ typedef struct {
     int32_t max_events;           /* capacity: events per call                                              */
     int64_t max_hits;             /* capacity: hits per call                                                */
     int32_t max_hits_per_event;   /* capacity: hits in one event (HOUGH_U16 needs <= 65535)                 */
-    int32_t flags;                /* reserved, 0                                                            */
+    int32_t flags;                /* 0 or HOUGH_FLAG_* bits                                                 */
     int32_t device;               /* CUDA device ordinal                                                    */
 } hough_plan_desc_t;
 
@@ -140,6 +146,11 @@ int hough_assign_hits(hough_plan_t* plan, const float* d_u, const float* d_v, co
 int hough_run_host(hough_plan_t* plan, const float* h_u, const float* h_v, const int64_t* h_offsets,
                    int32_t n_events, hough_candidate_t* h_cands, int32_t* h_n_found, int32_t* h_labels);
 
+/* The same with the number of chunks given (1 .. 32; 0 = automatic, about 24 M hits per chunk). */
+int hough_run_host_chunked(hough_plan_t* plan, const float* h_u, const float* h_v, const int64_t* h_offsets,
+                           int32_t n_events, hough_candidate_t* h_cands, int32_t* h_n_found, int32_t* h_labels,
+                           int32_t n_chunks);
+
 /* Derived constants; h_cos_q / h_sin_q are nullable host arrays of n_theta int32 that receive the tables. */
 int hough_plan_query(const hough_plan_t* plan, hough_plan_info_t* info, int32_t* h_cos_q, int32_t* h_sin_q);
 
@@ -151,7 +162,9 @@ int64_t hough_plan_launch_count(const hough_plan_t* plan);
 
 /* Diagnostic: reads and clears 16 per-phase SM-cycle sums (summed over CTAs) that the event kernel keeps only when
  * the library is built with -DHOUGH_PHASE_TIMERS; all zeros otherwise.  h_out16[15] is always the number of events the
- * last hough_find_clusters call on this plan handed from the fast kernel to the general kernel.  Synchronises `stream`. */
+ * last hough_find_clusters call on this plan handed from the fast kernel to the general kernel.  h_out16[14] / [13] are the
+ * number of failed index checks and the site code of the first one since the last call (always 0 unless the library is
+ * the -DHOUGH_BOUNDS debug build).  Synchronises `stream`. */
 int hough_plan_debug_counters(hough_plan_t* plan, uint64_t* h_out16, void* stream);
 
 /* Measures the conflict-free shared-memory atomic-add rate of the device (the roofline denominator of the

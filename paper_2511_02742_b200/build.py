@@ -16,7 +16,7 @@ SOURCES = [os.path.join(_HERE, "csrc", "hough_lib.cu")]
 DEPENDS = SOURCES + [os.path.join(_HERE, "csrc", "hough_kernels.cuh"), os.path.join(_HERE, "csrc", "hough_fast.cuh"), os.path.join(_ROOT, "include", "hough.h")]
 LIB = os.path.join(_HERE, "libhough.so")
 
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math",
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2,-Wall", "-shared", "-cudart", "static"]
 
 
@@ -27,23 +27,39 @@ def nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
-def is_stale() -> bool:
-    if not os.path.exists(LIB):
+# Debug variants: same sources, one extra define, their own file next to libhough.so.
+#   bounds  -DHOUGH_BOUNDS        every computed index inside the kernels is range-checked; a failed check sets
+#                                 HOUGH_STATUS_INTERNAL and skips the access (nothing is stored out of range, nothing traps)
+#   timers  -DHOUGH_PHASE_TIMERS  per-phase SM-cycle sums (hough_plan_debug_counters)
+VARIANTS = {"": [], "bounds": ["-DHOUGH_BOUNDS"], "timers": ["-DHOUGH_PHASE_TIMERS"]}
+
+
+def lib_path(variant: str = "") -> str:
+    return LIB if not variant else os.path.join(_HERE, f"libhough_{variant}.so")
+
+
+def is_stale(variant: str = "") -> bool:
+    lib = lib_path(variant)
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     return any(os.path.getmtime(d) > t for d in DEPENDS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not is_stale():
-        return LIB
-    tmp = LIB + f".tmp{os.getpid()}"
-    extra = os.environ.get("HOUGH_NVCC_EXTRA", "").split()      # e.g. -DHOUGH_PHASE_TIMERS for the diagnostic build
-    cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+def build(force: bool = False, verbose: bool = False, variant: str = "") -> str:
+    lib = lib_path(variant)
+    if not force and not is_stale(variant):
+        return lib
+    tmp = lib + f".tmp{os.getpid()}"
+    cmd = [nvcc()] + NVCC_FLAGS + VARIANTS[variant] + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
     subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    var = ""
+    for a in sys.argv[1:]:
+        if a.startswith("--variant="):
+            var = a.split("=", 1)[1]
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, variant=var))

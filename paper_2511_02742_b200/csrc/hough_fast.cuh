@@ -40,6 +40,7 @@ struct FastShared {  // static shared control block
     int n_on;     // on bins of the event so far (global on list)
     int n_peaks;  // peaks of the event so far
     int n_kept, n_ties;
+    int n_final;  // records of the event after selection (n_kept is still being read when this is written)
     int defer;
     int cstar, n_gt;  // threshold vote count and number of peaks above it
     unsigned int r2max;  // max over the event's valid hits of u_q^2 + v_q^2
@@ -47,9 +48,13 @@ struct FastShared {  // static shared control block
 
 __device__ __forceinline__ unsigned lanemask_lt()
 {
+#ifdef HOUGH_EMU
+    return (1u << (threadIdx.x & 31)) - 1u;
+#else
     unsigned m;
     asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
     return m;
+#endif
 }
 
 // Warp-aggregated append: every lane of the warp must call; returns the slot of this lane's item or -1.
@@ -72,11 +77,14 @@ __device__ __forceinline__ void split_L(const DevParams& P, uint32_t L, int& t, 
 }
 
 // union-find over on-list indices, 16-bit parents in shared memory (hook the larger root under the smaller one)
-__device__ __forceinline__ uint32_t suf_find(volatile unsigned short* parent, uint32_t x)
+__device__ __forceinline__ uint32_t suf_find(const DevParams& P, volatile unsigned short* parent, uint32_t x)
 {
+    if (!HB(P, x, P.f_oncap, 110)) return 0;
     uint32_t p = parent[x];
     while (p != x) {
+        if (!HB(P, p, P.f_oncap, 111)) return 0;
         const uint32_t gp = parent[p];
+        if (!HB(P, gp, P.f_oncap, 112)) return 0;
         if (gp == p) return p;
         parent[x] = (unsigned short)gp;  // path halving; x is not a root and never becomes one again
         x = gp;
@@ -85,11 +93,11 @@ __device__ __forceinline__ uint32_t suf_find(volatile unsigned short* parent, ui
     return x;
 }
 
-__device__ __forceinline__ void suf_union(unsigned short* parent, uint32_t a, uint32_t b)
+__device__ __forceinline__ void suf_union(const DevParams& P, unsigned short* parent, uint32_t a, uint32_t b)
 {
     while (true) {
-        a = suf_find(parent, a);
-        b = suf_find(parent, b);
+        a = suf_find(P, parent, a);
+        b = suf_find(P, parent, b);
         if (a == b) return;
         if (a < b) { const uint32_t t = a; a = b; b = t; }
         const unsigned short old = atomicCAS(parent + a, (unsigned short)a, (unsigned short)b);
@@ -108,14 +116,17 @@ __device__ __forceinline__ void suf_union(unsigned short* parent, uint32_t a, ui
     _Pragma("unroll") for (int g = 0; g < G; ++g) {                                                      \
         _Pragma("unroll") for (int j = 0; j < 2; ++j) {                                                  \
             const uint32_t a_ = (uint32_t)((HX) * C[g][j] + ((HY) * Sn[g][j] + Oq2));                    \
-            red_add_shared(((a_ >> sh) & amask) | col[g], j ? 0x10000u : 1u);                            \
+            const uint32_t ad_ = ((a_ >> sh) & amask) | col[g];                                          \
+            if (HB(P, ad_ - vt_base, vt_bytes, 101)) red_add_shared(ad_, j ? 0x10000u : 1u);             \
         }                                                                                                \
     }
 
 template <int G, int NW>
-__device__ __forceinline__ void fast_vote(const int2* __restrict__ hits, int n, int sh, uint32_t amask, int Oq2,
+__device__ __forceinline__ void fast_vote(const DevParams& P, uint32_t vt_base, const int2* __restrict__ hits, int n, int sh, uint32_t amask, int Oq2,
                                           const uint32_t (&col)[G], const int (&C)[G][2], const int (&Sn)[G][2])
 {
+    const uint32_t vt_bytes = (uint32_t)P.f_tile_bytes;  // used by the -DHOUGH_BOUNDS build only
+    (void)vt_base; (void)vt_bytes;
     // Hits are sliced over the NW warps of the CTA two at a time (one 16-byte broadcast load); a trip takes four such
     // pairs (the loads carry their strides as immediates), so the loop overhead is 7 instructions per 32 G votes.
     const int warp = threadIdx.x >> 5;
@@ -166,7 +177,7 @@ __device__ __forceinline__ void checked_vote(const DevParams& P, const int2* __r
             for (int j = 0; j < 2; ++j) {
                 const int a = h.x * C[g][j] + (h.y * Sn[g][j] + P.Oq);
                 const int r = a >> P.F;
-                if ((unsigned)r < n_rho && ((valid_bits >> (2 * g + j)) & 1u))
+                if ((unsigned)r < n_rho && ((valid_bits >> (2 * g + j)) & 1u) && HB(P, ((uint32_t)r << k) + col[g], P.f_tile_bytes, 102))
                     red_add_shared(tile_base + ((uint32_t)r << k) + col[g], j ? 0x10000u : 1u);
             }
     }
@@ -199,7 +210,7 @@ __global__ void __launch_bounds__(MAXT, MINB)
 hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* __restrict__ v,
                   const long long* __restrict__ offsets, int n_events, Candidate* __restrict__ cands, int* __restrict__ n_found)
 {
-    extern __shared__ __align__(1024) unsigned char smem[];
+    HOUGH_DYNAMIC_SMEM(smem);
     // the control block sits at the end of the dynamic allocation: no static shared memory, so the tile starts the window
     FastShared& sh = *reinterpret_cast<FastShared*>(smem + P.f_off_kept + (size_t)P.K * 20);
 
@@ -243,6 +254,11 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
     long long pt_last = clock64();
 #endif
 
+    // The address folding of the vote (Oq2) is valid only if the tile starts below 4096 in the shared window and on a row
+    // boundary (the host sized the fixed-point range for that).  If the driver ever places it elsewhere, nothing is
+    // computed here: every event this CTA fetches goes to the general kernel.
+    const bool fold_ok = tile_base < 4096u && (tile_base & ((1u << k) - 1u)) == 0u;
+
     while (true) {
         __syncthreads();  // previous event fully done
         if (tid == 0) {
@@ -255,7 +271,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 
         const long long g0 = offsets[e], g1 = offsets[e + 1];
         const long long ne64 = g1 - g0;
-        if (g0 < 0 || ne64 < 0 || ne64 > (long long)P.fHB || ne64 > (long long)P.max_hits_per_event) {
+        if (!fold_ok || g0 < 0 || ne64 < 0 || ne64 > (long long)P.fHB || ne64 > (long long)P.max_hits_per_event) {
             // bad offsets, or more hits than the staging buffer: the general kernel handles (and flags) it
             if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
             continue;
@@ -308,14 +324,18 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             if (strip == 0) {
                 // |u_q C + v_q S| <= (M + 1) sqrt(u_q^2 + v_q^2) for every theta (Cauchy-Schwarz; the table entries are within 1/2 of
                 // M cos, M sin), so all votes of the event fall into rows [(O_q - B) >> F, (O_q + B) >> F]
-                const long long B = (long long)P.Mq1 * ((long long)ceil(sqrt((double)sh.r2max)) + 1);
-                r_lo = (int)max(((long long)P.Oq - B) >> P.F, 0ll);
-                r_hi = (int)min(((long long)P.Oq + B) >> P.F, (long long)P.n_rho - 1);
+                // (stage_one clamps r2max at 2^32 - 1: a clamped value bounds nothing, every row stays reachable)
+                if (sh.r2max != 0xffffffffu) {
+                    const long long B = (long long)P.Mq1 * ((long long)ceil(sqrt((double)sh.r2max)) + 1);
+                    r_lo = (int)max(((long long)P.Oq - B) >> P.F, 0ll);
+                    r_hi = (int)min(((long long)P.Oq + B) >> P.F, (long long)P.n_rho - 1);
+                    if (r_lo > r_hi) { r_lo = 0; r_hi = P.n_rho - 1; }
+                }
             }
             HOUGH_PT(1);
             {
                 const int ns = sh.n_safe, nu = sh.n_unsafe;
-                if (full) fast_vote<G, MAXT / 32>(hits, ns, sh_reg, amask, Oq2, col, C, Sn);  // launched with MAXT threads
+                if (full) fast_vote<G, MAXT / 32>(P, tile_base, hits, ns, sh_reg, amask, Oq2, col, C, Sn);  // launched with MAXT threads
                 else checked_vote<G>(P, hits, 0, ns, tile_base, k, col, C, Sn, valid_bits);
                 if (nu) checked_vote<G>(P, hits, P.fHB - nu, nu, tile_base, k, col, C, Sn, valid_bits);
             }
@@ -334,9 +354,8 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 const uint32_t a_end = tile_base + 16u * (uint32_t)i_hi;
                 for (uint32_t a = tile_base + 16u * (uint32_t)(i_lo + tid); a - 16u * lane < a_end; a += 16u * nthr, hp += nthr / cpr) {
                     uint32_t m = 0;  // bit q set <=> count q of this chunk is on
-                    if (a < a_end) {
-                        uint4 w;
-                        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(a));
+                    if (a < a_end && HB(P, a - tile_base, P.f_tile_bytes, 122)) {
+                        const uint4 w = lds128(a);
                         // counts are below 2^15 (at most one vote per hit, fHB <= 32767), so adding 2^15 - T to both
                         // halfwords sets their top bits exactly where count >= T, without a carry between them
                         const uint32_t gx = (w.x + tadd) & 0x80008000u, gy = (w.y + tadd) & 0x80008000u;
@@ -348,7 +367,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                             if (((w.x + oadd) | (w.y + oadd) | (w.z + oadd) | (w.w + oadd)) & 0x80008000u) sh.defer = 1;
                         }
                         // theta rows beyond n_theta hold no votes (checked_vote masks them), so m needs no masking
-                        if (halo_lane) {  // the row's two last counts are the next strip's count halo
+                        if (halo_lane && HB(P, hp - halo_cur, P.n_rho, 120)) {  // the row's two last counts are the next strip's count halo
                             hp[0] = (uint16_t)(w.w & 0xffffu);  // (rows no vote can reach are never scanned: they stay 0 from the event's start)
                             hp[P.n_rho] = (uint16_t)(w.w >> 16);
                         }
@@ -358,7 +377,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     int cb = 0;
                     if (lane == 0) cb = atomicAdd(&sh.n_ch, __popc(bal));
                     cb = __shfl_sync(0xffffffffu, cb, 0) + __popc(bal & lanemask_lt());
-                    if (m != 0 && cb < P.fSLCAP) slist[P.fSLCAP - 1 - cb] = ((a - tile_base) >> 4) | (m << 16);
+                    if (m != 0 && cb < P.fSLCAP && HB(P, P.fSLCAP - 1 - cb, P.fSLCAP, 121)) slist[P.fSLCAP - 1 - cb] = ((a - tile_base) >> 4) | (m << 16);
                 }
             }
             __syncthreads();
@@ -375,7 +394,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 const int j = j0 + lane;
                 uint32_t m = 0, loc0 = 0, pk8 = 0;
                 uint4 Bw = make_uint4(0, 0, 0, 0);
-                if (j < n_ch) {
+                if (j < n_ch && HB(P, (slist[P.fSLCAP - 1 - j] & 0xffffu), P.f_tile_bytes >> 4, 123)) {
                     const uint32_t ce = slist[P.fSLCAP - 1 - j];
                     m = ce >> 16;
                     const int cidx = (int)(ce & 0xffffu);
@@ -432,7 +451,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     prev = (uint32_t)q;
                     const uint32_t c = (uint32_t)tile[loc0 + q] & kCountMax;
                     // strip-list entry: peak (bit 30) | offset back to its run's head (3 bits) | bin index inside the tile (17 bits) | votes (10 bits)
-                    if (slot < sl_lim) slist[slot] = (((pk8 >> q) & 1u) << 30) | (head << 27) | ((loc0 + q) << kCountBits) | c;
+                    if (slot < sl_lim && HB(P, slot, P.fSLCAP, 124)) slist[slot] = (((pk8 >> q) & 1u) << 30) | (head << 27) | ((loc0 + q) << kCountBits) | c;
                     ++slot;
                 }
             }
@@ -447,8 +466,9 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 const uint32_t ent = slist[i];
                 const uint32_t loc = (ent >> kCountBits) & 0x1ffffu;
                 const uint16_t en = (uint16_t)(kOnFlag | (uint32_t)(on0 + i));
+                if (!HB(P, loc, P.f_tile_bytes >> 1, 130) || !HB(P, on0 + i, P.f_oncap, 131)) continue;
                 tile[loc] = en;
-                if ((loc & (uint32_t)(S - 1)) == (uint32_t)(S - 1)) ihalo_cur[loc >> (k - 1)] = en;  // last theta row: index halo of the next strip
+                if ((loc & (uint32_t)(S - 1)) == (uint32_t)(S - 1) && HB(P, loc >> (k - 1), P.n_rho, 132)) ihalo_cur[loc >> (k - 1)] = en;  // last theta row: index halo of the next strip
                 parent[on0 + i] = (unsigned short)(on0 + i - (int)((ent >> 27) & 7u));  // the head of its run inside the chunk
             }
             __syncthreads();
@@ -459,6 +479,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             // strip list (this strip) or in the count halo (previous strip's last row).
             auto ncount = [&](uint32_t en, int tl_nb, int r_nb) -> uint32_t {
                 if (!(en & kOnFlag)) return 0u;
+                if (tl_nb >= 0 && !HB(P, (int)(en & 0x7fffu) - on0, n_sl, 140)) return 0u;
                 return tl_nb >= 0 ? (slist[(int)(en & 0x7fffu) - on0] & kCountMax) : (uint32_t)halo_prev[P.n_rho + r_nb];
             };
             // Lane l of a warp takes entry l * W + (warp-trip index): the 32 lanes of a warp work on 32 far-apart bins and do
@@ -497,13 +518,13 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 #pragma unroll 1
                 for (int kk = 0; kk < 2; ++kk) {
                     const uint32_t q = kk ? q1 : q0;
-                    if (q != 0xffffffffu) suf_union(parent, me_idx, q);
+                    if (q != 0xffffffffu && HB(P, q, on0 + n_sl, 141)) suf_union(P, parent, me_idx, q);
                     if (__ballot_sync(0xffffffffu, q1 != 0xffffffffu) == 0) break;  // warp-uniform
                 }
                 __syncwarp();  // reconverge after the data-dependent union loops
                 const int ip = warp_append(&sh.n_peaks, pk);
                 if (pk) {
-                    if (ip < P.fPCAP) { peaks[ip] = ((kCountMax - c) << kLBits) | L; pidx[ip] = (uint16_t)(on0 + i); }
+                    if (ip < P.fPCAP && HB(P, ip, P.fPCAP, 142)) { peaks[ip] = ((kCountMax - c) << kLBits) | L; pidx[ip] = (uint16_t)(on0 + i); }
                 }
                 hist_add(hist, pk, c);
             }
@@ -526,7 +547,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                     }
                     const int ip = warp_append(&sh.n_peaks, pk);
                     if (pk) {
-                        if (ip < P.fPCAP) {
+                        if (ip < P.fPCAP && HB(P, ip, P.fPCAP, 143)) {
                             peaks[ip] = ((kCountMax - c) << kLBits) | (uint32_t)((base - 1) * P.n_rho + r);
                             pidx[ip] = (uint16_t)(ihalo_prev[r] & 0x7fffu);
                         }
@@ -546,7 +567,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             continue;
         }
         // the tile is dead: its first ONCAP words become the root tags
-        for (int i = tid; i < n_on; i += nthr) roottag[i] = 0;
+        for (int i = tid; i < n_on; i += nthr) if (HB(P, i, P.f_tile_bytes >> 2, 150)) roottag[i] = 0;
 
         // ---------------- S4: the K best peaks (key = (1023 - votes) << 22 | L, ascending)
         if (n_pk > P.K) {
@@ -580,9 +601,9 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 int c = -1;
                 if (i < n_pk) { key = peaks[i]; c = (int)(kCountMax - (key >> kLBits)); }
                 const int a = warp_append(&sh.n_kept, c > cstar);
-                if (c > cstar) { kept[a] = key; kidx[a] = pidx[i]; }
+                if (c > cstar && HB(P, a, P.K, 151)) { kept[a] = key; kidx[a] = pidx[i]; }
                 const int b = warp_append(&sh.n_ties, c == cstar);
-                if (c == cstar && b < tcap) { tie_key[b] = key; tie_pos[b] = (uint32_t)i; }
+                if (c == cstar && b < tcap && HB(P, b, tcap, 152)) { tie_key[b] = key; tie_pos[b] = (uint32_t)i; }
             }
             __syncthreads();
             const int n_ties = sh.n_ties, n_gt = sh.n_kept;
@@ -595,21 +616,20 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                 const uint32_t key = tie_key[i];
                 int rank = 0;
                 for (int j = 0; j < n_ties; ++j) rank += (tie_key[j] < key);
-                if (rank < need) { kept[n_gt + rank] = key; kidx[n_gt + rank] = pidx[tie_pos[i]]; }
+                if (rank < need && HB(P, n_gt + rank, P.K, 153) && HB(P, tie_pos[i], P.fPCAP, 154)) { kept[n_gt + rank] = key; kidx[n_gt + rank] = pidx[tie_pos[i]]; }
             }
-            if (tid == 0) sh.n_kept = P.K;
+            if (tid == 0) sh.n_final = P.K;
         } else {
             for (int i = tid; i < n_pk; i += nthr) { kept[i] = peaks[i]; kidx[i] = pidx[i]; }
-            if (tid == 0) sh.n_kept = n_pk;
+            if (tid == 0) sh.n_final = n_pk;
         }
         __syncthreads();
-        const int n_kept = sh.n_kept;
+        const int n_kept = sh.n_final;
         for (int i = tid; i < n_kept; i += nthr) {  // slot = number of kept keys that are smaller (keys are unique)
             const uint32_t key = kept[i];
             int s = 0;
             for (int j = 0; j < n_kept; ++j) s += (kept[j] < key);
-            sorted[s] = key;
-            sidx[s] = kidx[i];
+            if (HB(P, s, P.K, 155)) { sorted[s] = key; sidx[s] = kidx[i]; }
             ksize[i] = 0;
         }
         __syncthreads();
@@ -617,17 +637,17 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 
         // ---------------- cluster of each kept peak: root, best-ranked kept peak of the same cluster, size
         for (int s = tid; s < n_kept; s += nthr) {
-            const uint32_t root = suf_find(parent, (uint32_t)sidx[s]);
+            const uint32_t root = suf_find(P, parent, (uint32_t)sidx[s]);
             kroot[s] = root;
-            atomicMax(roottag + root, (uint32_t)(P.K - s));  // the best-ranked (smallest slot) kept peak of the component wins
+            if (HB(P, root, n_on, 156)) atomicMax(roottag + root, (uint32_t)(P.K - s));  // the best-ranked (smallest slot) kept peak of the component wins
         }
         __syncthreads();
         HOUGH_PT(8);
         for (int i0 = tid - lane; i0 < n_on; i0 += nthr) {  // sizes of the components that own a kept peak
             const int i = i0 + lane;
             if (i < n_on) {
-                const uint32_t id = roottag[suf_find(parent, (uint32_t)i)];
-                if (id != 0) atomicAdd(ksize + (P.K - id), 1u);
+                const uint32_t id = roottag[suf_find(P, parent, (uint32_t)i)];
+                if (id != 0 && HB(P, P.K - id, P.K, 157)) atomicAdd(ksize + (P.K - id), 1u);
             }
             __syncwarp();
         }
@@ -639,7 +659,8 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             const uint32_t key = sorted[s];
             const uint32_t L = key & kLMask;
             const uint32_t c = kCountMax - (key >> kLBits);
-            const int rs = P.K - (int)roottag[kroot[s]];
+            int rs = P.K - (int)roottag[kroot[s]];
+            if (!HB(P, rs, n_kept, 158)) rs = 0;
             int t, r;
             split_L(P, L, t, r);
             const float th = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)t), (double)P.n_theta);

@@ -11,7 +11,13 @@
 // The accumulator never leaves shared memory on this path; an accumulator larger than shared memory is
 // processed as strips of theta rows (votes are separable per theta row).
 #pragma once
+#ifdef HOUGH_EMU  // host model of the CUDA execution for the CPU tests (tests/emu/cuda_emu.h); never defined in the product build
+#include "cuda_emu.h"
+#define HOUGH_DYNAMIC_SMEM(name_) unsigned char* name_ = cuda_emu::g_smem
+#else
 #include <cuda_runtime.h>
+#define HOUGH_DYNAMIC_SMEM(name_) extern __shared__ __align__(1024) unsigned char name_[]
+#endif
 #include <stdint.h>
 
 namespace hough {
@@ -25,6 +31,23 @@ namespace hough {
     } while (0)
 #else
 #define HOUGH_PT(k) do { } while (0)
+#endif
+
+// Debug-bounds build (-DHOUGH_BOUNDS): every computed shared-memory / scratch index is range-checked before the access;
+// a violation sets HOUGH_STATUS_INTERNAL (bit 2 of the status word), counts itself, records its site, and the access is
+// skipped -- nothing is stored out of range and nothing traps.  HB(...) is `true` in the product build.
+constexpr int kStatusInternal = 4;
+#ifdef HOUGH_BOUNDS
+__device__ __noinline__ bool hb_fail(int* status, int site)
+{
+    atomicOr(status, kStatusInternal);
+    atomicAdd(status + 2, 1);           // number of violations
+    atomicCAS(status + 1, 0, site);     // first site seen
+    return false;
+}
+#define HB(P_, i_, cap_, site_) (((unsigned long long)(long long)(i_) < (unsigned long long)(long long)(cap_)) ? true : hough::hb_fail((P_).status, (site_)))
+#else
+#define HB(P_, i_, cap_, site_) true
 #endif
 
 constexpr int kLBits = 22;                       // linear bin index L = t * n_rho + r < 2^22
@@ -80,7 +103,23 @@ __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)
 
 __device__ __forceinline__ void red_add_shared(uint32_t addr, uint32_t v)
 {
+#ifdef HOUGH_EMU
+    if (uint32_t* w = static_cast<uint32_t*>(emu_shared_ptr(addr, 4, "red.shared.add.u32 outside the CTA's shared memory"))) *w += v;
+#else
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+#endif
+}
+
+__device__ __forceinline__ uint4 lds128(uint32_t addr)
+{
+    uint4 w;
+#ifdef HOUGH_EMU
+    const uint4* q = static_cast<const uint4*>(emu_shared_ptr(addr, 16, "ld.shared.v4.u32 outside the CTA's shared memory"));
+    w = q ? *q : make_uint4(0, 0, 0, 0);
+#else
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(addr));
+#endif
+    return w;
 }
 
 __device__ __forceinline__ uint64_t mix64(uint64_t x)
@@ -137,9 +176,11 @@ __device__ __forceinline__ void stage_one(const DevParams& P, const StageCtx& sc
     const unsigned long long r2 = (unsigned long long)((long long)uq * uq) + (unsigned long long)((long long)vq * vq);
     r2loc = max(r2loc, r2 > 0xffffffffull ? 0xffffffffu : (unsigned int)r2);
     if (P.safe_enabled && r2 <= P.r2safe) {
-        sc.hits[atomicAdd(sc.n_safe, 1)] = make_int2(uq, vq);
+        const int i = atomicAdd(sc.n_safe, 1);
+        if (HB(P, i, sc.hb, 100)) sc.hits[i] = make_int2(uq, vq);
     } else {
-        sc.hits[sc.hb - 1 - atomicAdd(sc.n_unsafe, 1)] = make_int2(uq, vq);
+        const int i = sc.hb - 1 - atomicAdd(sc.n_unsafe, 1);
+        if (HB(P, i, sc.hb, 100)) sc.hits[i] = make_int2(uq, vq);
     }
 }
 
@@ -192,7 +233,7 @@ __device__ __forceinline__ void vote_hits(const DevParams& P, const int2* __rest
             for (int j = 0; j < TPW; ++j) {
                 const int a = h.x * C[g][j] + (h.y * Sn[g][j] + (CHECK ? O[g][j] : P.Oq));
                 const int r = a >> F;  // floor(a / 2^F)
-                if (!CHECK || (unsigned)r < n_rho) {
+                if ((!CHECK || (unsigned)r < n_rho) && HB(P, r, n_rho, 200)) {
                     const uint32_t addr = colbase + (uint32_t)(r * rb);
                     red_add_shared(addr + 128u * g, (CW == 2 && j == 1) ? 0x10000u : 1u);
                 }
@@ -256,7 +297,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
     // with an event list, the kernel processes events event_list[0 .. *event_list_count) instead of 0 .. n_events
     if (event_list) n_events = (int)*event_list_count;
     constexpr int TPW = 4 / CW;
-    extern __shared__ __align__(1024) unsigned char smem[];
+    HOUGH_DYNAMIC_SMEM(smem);
     __shared__ EventShared sh;
 
     unsigned char* tile = smem;
@@ -415,6 +456,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
                         const int tl = q * 4 * TPW + k;
                         const uint32_t L = (uint32_t)((base + tl) * P.n_rho + r);
                         const int io = atomicAdd(&sh.n_on, 1);
+                        if (!HB(P, io, P.n_bins, 201) || !HB(P, L, P.n_bins, 202)) continue;
                         __stcg(onlist + io, make_uint2(L, c));
                         __stcg(parent + L, tag | L);
                         __stcg(csize + L, 0u);
@@ -525,7 +567,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
         HOUGH_PT(8);
         for (int i = tid; i < n_pk; i += nthr) {
             const unsigned long long k = peak_key(i);
-            if (k <= kth) kept[atomicAdd(&sh.n_kept, 1)] = k;
+            if (k <= kth) { const int ik = atomicAdd(&sh.n_kept, 1); if (HB(P, ik, P.K, 203)) kept[ik] = k; }
         }
         __syncthreads();  // also orders the csize atomics before the reads below
         const int n_kept = sh.n_kept;
@@ -535,7 +577,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
             const unsigned long long k = kept[i];
             int s = 0;
             for (int j = 0; j < n_kept; ++j) s += (kept[j] < k);
-            sorted[s] = k;
+            if (HB(P, s, P.K, 204)) sorted[s] = k;
         }
         __syncthreads();
         for (int s = tid; s < n_kept; s += nthr) kroot[s] = uf_find(parent, (uint32_t)(sorted[s] & 0xffffffffULL), tag);
@@ -546,7 +588,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
             const uint32_t c = ~(uint32_t)(k >> 32);
             const uint32_t root = kroot[s];
             int rs = 0;
-            while (kroot[rs] != root) ++rs;  // best-ranked kept peak of the same component (<= s)
+            while (rs < s && kroot[rs] != root) ++rs;  // best-ranked kept peak of the same component (<= s)
             Candidate cd;
             cd.theta_bin = (int)(L / (uint32_t)P.n_rho);
             cd.rho_bin = (int)(L - (uint32_t)cd.theta_bin * P.n_rho);
@@ -580,7 +622,7 @@ hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float*
                     const long long* __restrict__ offsets, int n_events, const Candidate* __restrict__ cands,
                     const int* __restrict__ n_found, int* __restrict__ labels)
 {
-    extern __shared__ __align__(1024) unsigned char smem[];
+    HOUGH_DYNAMIC_SMEM(smem);
     int4* trip = reinterpret_cast<int4*>(smem);  // [K]
     const int tid = threadIdx.x, nthr = blockDim.x;
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
@@ -641,7 +683,7 @@ hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float*
 __global__ void __launch_bounds__(1024, 1)
 smem_atomic_peak_kernel(int iters, int rows, unsigned long long* cycles, uint32_t* sink)
 {
-    extern __shared__ __align__(1024) unsigned char smem[];
+    HOUGH_DYNAMIC_SMEM(smem);
     uint32_t* w = reinterpret_cast<uint32_t*>(smem);
     const int lane = threadIdx.x & 31;
     for (int i = threadIdx.x; i < rows * 32; i += blockDim.x) w[i] = 0;
@@ -657,7 +699,7 @@ smem_atomic_peak_kernel(int iters, int rows, unsigned long long* cycles, uint32_
     const long long t0 = clock64();
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
-        for (int j = 0; j < 16; ++j) asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a[j]), "r"((j & 1) ? 0x10000u : 1u));
+        for (int j = 0; j < 16; ++j) red_add_shared(a[j], (j & 1) ? 0x10000u : 1u);
     }
     const long long t1 = clock64();
     __syncthreads();

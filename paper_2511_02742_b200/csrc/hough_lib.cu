@@ -19,6 +19,14 @@ using hough::DevParams;
 static_assert(sizeof(hough_candidate_t) == 32, "record layout");
 static_assert(sizeof(Candidate) == sizeof(hough_candidate_t), "device record mirrors the ABI record");
 
+// kernel launch: the <<< >>> syntax, or the host model of tests/emu when the sources are compiled for the CPU tests
+#ifdef HOUGH_EMU
+#define HOUGH_LAUNCH(kernel_, grid_, block_, smem_, stream_, ...) \
+    cuda_emu::launch(dim3(grid_), dim3(block_), (size_t)(smem_), [&]() { kernel_(__VA_ARGS__); })
+#else
+#define HOUGH_LAUNCH(kernel_, grid_, block_, smem_, stream_, ...) kernel_<<<(grid_), (block_), (smem_), (stream_)>>>(__VA_ARGS__)
+#endif
+
 static thread_local char g_cuda_err[256] = "";
 
 static int cuda_fail(cudaError_t e, const char* what)
@@ -56,6 +64,7 @@ struct hough_plan {
     int* d_status;
     unsigned int* d_counter;
     // lazily created resources of hough_run_host
+    bool h_ready;                        // every resource below exists
     cudaStream_t h_stream;               // compute stream of hough_run_host
     cudaStream_t h_up, h_down;           // copy streams: host -> device, device -> host
     cudaEvent_t h_ev_up[kHostChunksMax], h_ev_done[kHostChunksMax];
@@ -67,11 +76,17 @@ struct hough_plan {
     int* hd_labels;
 };
 
+// Experiment switches exist only in the tuning build (-DHOUGH_TUNING, used from _work/): the results and the launch
+// shape of the product library never depend on the environment of the calling process.
+#ifdef HOUGH_TUNING
 static int env_int(const char* name, int dflt)
 {
     const char* s = getenv(name);
     return (s && *s) ? atoi(s) : dflt;
 }
+#else
+static inline int env_int(const char*, int dflt) { return dflt; }
+#endif
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
@@ -103,7 +118,7 @@ static cudaError_t launch_event_kernel(const hough_plan* p, const float* u, cons
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
-    k<<<p->n_ctas, p->threads, p->smem_bytes, st>>>(p->P, u, v, off, n_events, cands, n_found, acc, acc_u16, digest, elist, ecount);
+    HOUGH_LAUNCH(k, p->n_ctas, p->threads, p->smem_bytes, st, p->P, u, v, off, n_events, cands, n_found, acc, acc_u16, digest, elist, ecount);
     return cudaGetLastError();
 }
 
@@ -133,22 +148,7 @@ static cudaError_t launch_fast(const hough_plan* p, const float* u, const float*
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
-    if (getenv("HOUGH_DEBUG_OCCUPANCY")) {
-        int occ = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, p->f_threads, p->f_smem);
-        cudaFuncAttributes fa;
-        cudaFuncGetAttributes(&fa, k);
-        cudaDeviceProp prop;
-        cudaGetDeviceProperties(&prop, p->desc.device);
-        fprintf(stderr, "hough_fast_kernel<%d,%d,%d>: %d threads, %d B dynamic smem -> %d CTAs/SM (regs %d, static smem %zu, local %zu; SM smem %zu, "
-                        "reserved/block %zu, regs/SM %d)\n", G, MAXT, MINB, p->f_threads, p->f_smem, occ, fa.numRegs, fa.sharedSizeBytes,
-                fa.localSizeBytes, prop.sharedMemPerMultiprocessor, prop.reservedSharedMemPerBlock, prop.regsPerMultiprocessor);
-        for (int sm = p->f_smem; sm > p->f_smem - 8192; sm -= 512) {
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, p->f_threads, sm);
-            if (occ >= 2) { fprintf(stderr, "  2 CTAs/SM fit at %d B dynamic smem\n", sm); break; }
-        }
-    }
-    k<<<p->f_ctas, p->f_threads, p->f_smem, st>>>(p->P, u, v, off, n_events, cands, n_found);
+    HOUGH_LAUNCH(k, p->f_ctas, p->f_threads, p->f_smem, st, p->P, u, v, off, n_events, cands, n_found);
     return cudaGetLastError();
 }
 
@@ -188,7 +188,9 @@ static FastLayout layout_fast(int tile_bytes, int HB, int n_rho, int SLCAP, int 
 
 extern "C" {
 
-int hough_version(void) { return 100; }
+static void free_host_path(hough_plan_t* p);
+
+int hough_version(void) { return 200; }
 
 const char* hough_strerror(int s)
 {
@@ -213,6 +215,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     if (d->max_candidates < 1 || d->max_candidates > 4096) return HOUGH_EINVAL;
     if (d->count_dtype != HOUGH_I32 && d->count_dtype != HOUGH_U16) return HOUGH_EINVAL;
     if (d->max_events < 1 || d->max_hits < 0 || d->max_hits_per_event < 0 || d->device < 0) return HOUGH_EINVAL;
+    if (d->flags & ~(HOUGH_FLAG_GENERAL_ONLY | HOUGH_FLAG_SMALL_LISTS)) return HOUGH_EINVAL;
     if (d->count_dtype == HOUGH_U16 && d->max_hits_per_event > 65535) return HOUGH_ERANGE;  // a bin gets <= 1 vote per hit
     if ((int64_t)d->n_theta * d->n_rho > (1ll << hough::kLBits)) return HOUGH_ERANGE;
     const int H = d->hit_frac_bits < 0 ? 6 : d->hit_frac_bits;
@@ -325,7 +328,10 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     p->f_G = 0;
     FastLayout flay{};
     int f_S = 0, f_nstrips = 0, f_tile = 0, f_HB = 0, f_SLCAP = 0, f_PCAP = 0, f_ONCAP = 0, f_k = 0;
-    if (cw == 2 && d->vote_threshold <= 1023 && K <= 1000 && d->max_hits_per_event >= 1 && !env_int("HOUGH_NO_FAST", 0)) {
+    if (cw == 2 && d->vote_threshold <= 1023 && K <= 1000 && d->max_hits_per_event >= 1 && !env_int("HOUGH_NO_FAST", 0) &&
+        !(d->flags & HOUGH_FLAG_GENERAL_ONLY) &&
+        // the reachable-row bound of the fast kernel keeps u_q^2 + v_q^2 in 32 bits
+        2.0 * (double)qmax * (double)qmax <= 4294967295.0) {
         struct Cand { int G, maxt, minb, threads, cps; };
         // preference order: one 1024-thread CTA per SM with the widest tile row that fits, then two CTAs per SM
         const Cand cands[] = {{4, 1024, 1, 1024, 1}, {2, 1024, 1, 1024, 1}, {1, 1024, 1, 1024, 1}, {4, 768, 2, 768, 2}, {2, 768, 2, 768, 2}, {1, 768, 2, 768, 2}};
@@ -349,6 +355,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
             // the strip list also holds the strip's on-chunk list at its end (hough_fast.cuh S2)
             int slcap = env_int("HOUGH_FAST_SLCAP", 2560 * c.G > 10240 ? 10240 : 2560 * c.G), pcap = env_int("HOUGH_FAST_PCAP", 3584);
             int oncap = env_int("HOUGH_FAST_ONCAP", 12288);
+            if (d->flags & HOUGH_FLAG_SMALL_LISTS) { slcap = 64; pcap = 4; oncap = 16; }  // events overflow and are deferred
             if (oncap > 32767) oncap = 32767;
             if (oncap * 4 > tile) oncap = tile / 4;  // root tags reuse the tile
             auto total = [&]() { return layout_fast(tile, hb, d->n_rho, slcap, pcap, oncap, K).total; };
@@ -476,16 +483,7 @@ int hough_plan_destroy(hough_plan_t* p)
     (void)cudaDeviceSynchronize();
     cudaFree(p->d_cos); cudaFree(p->d_sin); cudaFree(p->d_scratch); cudaFree(p->d_status);
     cudaFree(p->d_fcos); cudaFree(p->d_fsin); cudaFree(p->d_deferred);
-    cudaFree(p->hd_u); cudaFree(p->hd_v); cudaFree(p->hd_off); cudaFree(p->hd_cands); cudaFree(p->hd_nfound); cudaFree(p->hd_labels);
-    if (p->h_stream) {
-        cudaStreamDestroy(p->h_stream);
-        if (p->h_up) cudaStreamDestroy(p->h_up);
-        if (p->h_down) cudaStreamDestroy(p->h_down);
-        for (int c = 0; c < kHostChunksMax; ++c) {
-            if (p->h_ev_up[c]) cudaEventDestroy(p->h_ev_up[c]);
-            if (p->h_ev_done[c]) cudaEventDestroy(p->h_ev_done[c]);
-        }
-    }
+    free_host_path(p);
     (void)cudaGetLastError();
     delete p;
     return HOUGH_OK;
@@ -513,6 +511,12 @@ int hough_plan_debug_counters(hough_plan_t* p, uint64_t* h_out16, void* stream)
     HCK(cudaMemcpyAsync(&deferred, p->P.deferred_count, sizeof deferred, cudaMemcpyDeviceToHost, st));
     HCK(cudaStreamSynchronize(st));
     h_out16[15] = deferred;
+    int st3[3] = {0, 0, 0};  // status word, first violation site, violation count (-DHOUGH_BOUNDS build; zeros otherwise)
+    HCK(cudaMemcpyAsync(st3, p->d_status, sizeof st3, cudaMemcpyDeviceToHost, st));
+    HCK(cudaMemsetAsync(p->d_status + 1, 0, 2 * sizeof(int), st));
+    HCK(cudaStreamSynchronize(st));
+    h_out16[13] = (uint64_t)(uint32_t)st3[1];
+    h_out16[14] = (uint64_t)(uint32_t)st3[2];
     return HOUGH_OK;
 }
 
@@ -590,16 +594,58 @@ int hough_assign_hits(hough_plan_t* p, const float* d_u, const float* d_v, const
     const int grid = n_events < p->assign_ctas ? n_events : p->assign_ctas;
     if ((size_t)p->P.K * 16 > 48 * 1024)
         HCK(cudaFuncSetAttribute(hough::hough_assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, p->P.K * 16));
-    hough::hough_assign_kernel<<<grid, 256, (size_t)p->P.K * 16, st>>>(p->P, d_u, d_v, reinterpret_cast<const long long*>(d_offsets),
-                                                                      n_events, reinterpret_cast<const Candidate*>(d_cands),
-                                                                      d_n_found, d_labels);
+    HOUGH_LAUNCH(hough::hough_assign_kernel, grid, 256, (size_t)p->P.K * 16, st, p->P, d_u, d_v, reinterpret_cast<const long long*>(d_offsets),
+                 n_events, reinterpret_cast<const Candidate*>(d_cands), d_n_found, d_labels);
     HCK(cudaGetLastError());
     p->launches += 1;
     return HOUGH_OK;
 }
 
+static void free_host_path(hough_plan_t* p)
+{
+    cudaFree(p->hd_u); cudaFree(p->hd_v); cudaFree(p->hd_off); cudaFree(p->hd_cands); cudaFree(p->hd_nfound); cudaFree(p->hd_labels);
+    p->hd_u = p->hd_v = nullptr; p->hd_off = nullptr; p->hd_cands = nullptr; p->hd_nfound = p->hd_labels = nullptr;
+    if (p->h_stream) cudaStreamDestroy(p->h_stream);
+    if (p->h_up) cudaStreamDestroy(p->h_up);
+    if (p->h_down) cudaStreamDestroy(p->h_down);
+    p->h_stream = p->h_up = p->h_down = nullptr;
+    for (int c = 0; c < kHostChunksMax; ++c) {
+        if (p->h_ev_up[c]) cudaEventDestroy(p->h_ev_up[c]);
+        if (p->h_ev_done[c]) cudaEventDestroy(p->h_ev_done[c]);
+        p->h_ev_up[c] = p->h_ev_done[c] = nullptr;
+    }
+    p->h_ready = false;
+    (void)cudaGetLastError();
+}
+
+static int init_host_path(hough_plan_t* p)
+{
+    const size_t mh = (size_t)(p->desc.max_hits > 0 ? p->desc.max_hits : 1) + 4, me = (size_t)p->desc.max_events;
+    HCK(cudaStreamCreateWithFlags(&p->h_stream, cudaStreamNonBlocking));
+    HCK(cudaStreamCreateWithFlags(&p->h_up, cudaStreamNonBlocking));
+    HCK(cudaStreamCreateWithFlags(&p->h_down, cudaStreamNonBlocking));
+    for (int c = 0; c < kHostChunksMax; ++c) {
+        HCK(cudaEventCreateWithFlags(&p->h_ev_up[c], cudaEventDisableTiming));
+        HCK(cudaEventCreateWithFlags(&p->h_ev_done[c], cudaEventDisableTiming));
+    }
+    HCK(cudaMalloc((void**)&p->hd_u, mh * 4));
+    HCK(cudaMalloc((void**)&p->hd_v, mh * 4));
+    HCK(cudaMalloc((void**)&p->hd_off, (me + 1) * 8));
+    HCK(cudaMalloc((void**)&p->hd_cands, me * p->desc.max_candidates * sizeof(Candidate)));
+    HCK(cudaMalloc((void**)&p->hd_nfound, me * 4));
+    HCK(cudaMalloc((void**)&p->hd_labels, mh * 4));
+    HCK(cudaMemset(p->hd_cands, 0, me * p->desc.max_candidates * sizeof(Candidate)));  // rows beyond n_found read as zeros
+    return HOUGH_OK;
+}
+
 int hough_run_host(hough_plan_t* p, const float* h_u, const float* h_v, const int64_t* h_offsets, int32_t n_events,
                    hough_candidate_t* h_cands, int32_t* h_n_found, int32_t* h_labels)
+{
+    return hough_run_host_chunked(p, h_u, h_v, h_offsets, n_events, h_cands, h_n_found, h_labels, 0);
+}
+
+int hough_run_host_chunked(hough_plan_t* p, const float* h_u, const float* h_v, const int64_t* h_offsets, int32_t n_events,
+                           hough_candidate_t* h_cands, int32_t* h_n_found, int32_t* h_labels, int32_t n_chunks)
 {
     if (!p || !h_offsets || n_events < 0) return HOUGH_EINVAL;
     if (n_events > p->desc.max_events) return HOUGH_ERANGE;
@@ -609,27 +655,15 @@ int hough_run_host(hough_plan_t* p, const float* h_u, const float* h_v, const in
     if (n_hits < 0 || (n_hits > 0 && (!h_u || !h_v))) return HOUGH_EINVAL;
     if (n_hits > p->desc.max_hits) return HOUGH_ERANGE;
     HCK(cudaSetDevice(p->desc.device));
-    if (!p->h_stream) {
-        const size_t mh = (size_t)(p->desc.max_hits > 0 ? p->desc.max_hits : 1) + 4, me = (size_t)p->desc.max_events;
-        HCK(cudaStreamCreateWithFlags(&p->h_stream, cudaStreamNonBlocking));
-        HCK(cudaStreamCreateWithFlags(&p->h_up, cudaStreamNonBlocking));
-        HCK(cudaStreamCreateWithFlags(&p->h_down, cudaStreamNonBlocking));
-        for (int c = 0; c < kHostChunksMax; ++c) {
-            HCK(cudaEventCreateWithFlags(&p->h_ev_up[c], cudaEventDisableTiming));
-            HCK(cudaEventCreateWithFlags(&p->h_ev_done[c], cudaEventDisableTiming));
-        }
-        HCK(cudaMalloc((void**)&p->hd_u, mh * 4));
-        HCK(cudaMalloc((void**)&p->hd_v, mh * 4));
-        HCK(cudaMalloc((void**)&p->hd_off, (me + 1) * 8));
-        HCK(cudaMalloc((void**)&p->hd_cands, me * p->desc.max_candidates * sizeof(Candidate)));
-        HCK(cudaMalloc((void**)&p->hd_nfound, me * 4));
-        HCK(cudaMalloc((void**)&p->hd_labels, mh * 4));
-        HCK(cudaMemset(p->hd_cands, 0, me * p->desc.max_candidates * sizeof(Candidate)));  // rows beyond n_found read as zeros
+    if (n_chunks < 0) return HOUGH_EINVAL;
+    if (!p->h_ready) {  // lazily created; flagged ready only when every stream, event and buffer exists
+        const int rc = init_host_path(p);
+        if (rc != HOUGH_OK) { free_host_path(p); return rc; }
+        p->h_ready = true;
     }
     // The batch is cut into chunks of events with about equal hit counts; chunk c's hits go up on one stream while chunk
     // c - 1 is computed on a second and chunk c - 2's results come down on a third (PCIe is full duplex).  The kernels of all
     // chunks run on ONE stream, in order: the plan's counters and scratch are not shared between concurrent launches.
-    int n_chunks = env_int("HOUGH_HOST_CHUNKS", 0);
     if (n_chunks <= 0) n_chunks = (int)(n_hits / (24ll << 20)) + 1;  // ~24 M hits (200 MB of input) per chunk
     if (n_chunks > kHostChunksMax) n_chunks = kHostChunksMax;
     if (n_chunks > n_events) n_chunks = n_events;
@@ -699,7 +733,7 @@ int hough_measure_smem_atomic_peak(int32_t device, double millis, double* ops_pe
     float ms = 0;
     for (int pass = 0; pass < 3; ++pass) {  // warm-up, calibration, measurement
         HCK(cudaEventRecord(e0));
-        hough::smem_atomic_peak_kernel<<<grid, threads, sm>>>(iters, rows, d_cyc, d_sink);
+        HOUGH_LAUNCH(hough::smem_atomic_peak_kernel, grid, threads, sm, (cudaStream_t)0, iters, rows, d_cyc, d_sink);
         HCK(cudaGetLastError());
         HCK(cudaEventRecord(e1));
         HCK(cudaEventSynchronize(e1));

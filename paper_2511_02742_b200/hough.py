@@ -23,7 +23,8 @@ LIB_PATH = os.path.join(_HERE, "libhough.so")
 
 HOUGH_OK, HOUGH_EINVAL, HOUGH_ERANGE, HOUGH_ECUDA, HOUGH_ENOMEM = 0, -1, -2, -3, -4
 HOUGH_I32, HOUGH_U16 = 0, 1
-HOUGH_STATUS_EVENT_TOO_LONG, HOUGH_STATUS_BAD_OFFSETS = 1, 2
+HOUGH_STATUS_EVENT_TOO_LONG, HOUGH_STATUS_BAD_OFFSETS, HOUGH_STATUS_INTERNAL = 1, 2, 4
+HOUGH_FLAG_GENERAL_ONLY, HOUGH_FLAG_SMALL_LISTS = 1, 2
 
 # numpy view of hough_candidate_t (32 bytes)
 CANDIDATE_DTYPE = np.dtype([("theta_bin", "<i4"), ("rho_bin", "<i4"), ("votes", "<i4"), ("cluster_root", "<i4"),
@@ -31,7 +32,7 @@ CANDIDATE_DTYPE = np.dtype([("theta_bin", "<i4"), ("rho_bin", "<i4"), ("votes", 
 CANDIDATE_WORDS = 8   # a record is 8 x 32-bit words; device tensors of records are int32 [E, K, 8]
 
 EXPORTS = ("hough_plan_create", "hough_plan_destroy", "hough_vote", "hough_find_clusters", "hough_assign_hits",
-           "hough_run_host", "hough_plan_query", "hough_plan_status", "hough_plan_launch_count", "hough_plan_debug_counters",
+           "hough_run_host", "hough_run_host_chunked", "hough_plan_query", "hough_plan_status", "hough_plan_launch_count", "hough_plan_debug_counters",
            "hough_measure_smem_atomic_peak", "hough_strerror", "hough_last_cuda_error", "hough_version")
 
 
@@ -81,6 +82,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     L.hough_find_clusters.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp]
     L.hough_assign_hits.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp, vp]
     L.hough_run_host.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp]
+    L.hough_run_host_chunked.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp, i32]
     L.hough_plan_query.argtypes = [vp, ctypes.POINTER(hough_plan_info_t), vp, vp]
     L.hough_plan_status.argtypes = [vp, ctypes.POINTER(i32), vp]
     L.hough_plan_launch_count.argtypes = [vp]
@@ -122,10 +124,11 @@ class Plan:
 
 def hough_plan_create(n_theta: int, n_rho: int, rho_min: float, rho_max: float, coord_max: float, vote_threshold: int,
                       assign_window: float, max_candidates: int, max_events: int, max_hits: int, max_hits_per_event: int,
-                      count_dtype: int = HOUGH_I32, hit_frac_bits: int = -1, acc_frac_bits: int = -1, device: int = 0) -> Plan:
+                      count_dtype: int = HOUGH_I32, hit_frac_bits: int = -1, acc_frac_bits: int = -1, device: int = 0,
+                      flags: int = 0) -> Plan:
     L = load_library()
     d = hough_plan_desc_t(n_theta, n_rho, rho_min, rho_max, coord_max, hit_frac_bits, acc_frac_bits, vote_threshold,
-                          assign_window, max_candidates, count_dtype, max_events, max_hits, max_hits_per_event, 0, device)
+                          assign_window, max_candidates, count_dtype, max_events, max_hits, max_hits_per_event, flags, device)
     h = ctypes.c_void_p()
     _check(L.hough_plan_create(ctypes.byref(d), ctypes.byref(h)), "hough_plan_create")
     return Plan(h.value, d)
@@ -157,7 +160,9 @@ def hough_plan_launch_count(plan: Plan) -> int:
 
 
 def hough_plan_debug_counters(plan: Plan, stream=None) -> np.ndarray:
-    """uint64 [16] per-phase SM-cycle sums (zeros unless libhough was built with -DHOUGH_PHASE_TIMERS); clears them."""
+    """uint64 [16]: per-phase SM-cycle sums (zeros unless libhough was built with -DHOUGH_PHASE_TIMERS; cleared);
+    [15] = events the last hough_find_clusters call deferred from the fast to the general kernel; [14], [13] = failed
+    index checks and the first failing site (only the -DHOUGH_BOUNDS build can report non-zero)."""
     out = np.zeros(16, np.uint64)
     _check(load_library().hough_plan_debug_counters(plan.handle, out.ctypes.data, _stream_ptr(plan, stream)),
            "hough_plan_debug_counters")
@@ -238,15 +243,27 @@ def _host(t, dtype, name):
     return ctypes.c_void_p(t.data_ptr())
 
 
-def hough_run_host(plan: Plan, u, v, offsets, cands, n_found, labels) -> None:
+def hough_run_host(plan: Plan, u, v, offsets, cands, n_found, labels, n_chunks: int = 0) -> None:
     """Whole pipeline on HOST buffers (numpy arrays or CPU torch tensors, ideally pinned); outputs are filled in place.
-    cands: int32 [E, K, 8] (or CANDIDATE_DTYPE [E, K]); n_found int32 [E]; labels int32 [N]; any output may be None."""
+    cands: int32 [E, K, 8] (or CANDIDATE_DTYPE [E, K]); n_found int32 [E]; labels int32 [N]; any output may be None.
+    n_chunks > 0 calls hough_run_host_chunked with that many chunks."""
     E = int(offsets.shape[0]) - 1
+    if n_chunks:
+        return hough_run_host_chunked(plan, u, v, offsets, cands, n_found, labels, n_chunks)
     _check(load_library().hough_run_host(plan.handle, _host(u, np.float32, "u"), _host(v, np.float32, "v"),
                                          _host(offsets, np.int64, "offsets"), E,
                                          None if cands is None else ctypes.c_void_p(cands.ctypes.data if isinstance(cands, np.ndarray) else cands.data_ptr()),
                                          None if n_found is None else _host(n_found, np.int32, "n_found"),
                                          None if labels is None else _host(labels, np.int32, "labels")), "hough_run_host")
+
+
+def hough_run_host_chunked(plan: Plan, u, v, offsets, cands, n_found, labels, n_chunks: int) -> None:
+    E = int(offsets.shape[0]) - 1
+    _check(load_library().hough_run_host_chunked(
+        plan.handle, _host(u, np.float32, "u"), _host(v, np.float32, "v"), _host(offsets, np.int64, "offsets"), E,
+        None if cands is None else ctypes.c_void_p(cands.ctypes.data if isinstance(cands, np.ndarray) else cands.data_ptr()),
+        None if n_found is None else _host(n_found, np.int32, "n_found"),
+        None if labels is None else _host(labels, np.int32, "labels"), int(n_chunks)), "hough_run_host_chunked")
 
 
 def hough_measure_smem_atomic_peak(device: int = 0, millis: float = 20.0) -> Tuple[float, float]:
@@ -267,8 +284,8 @@ def candidates_to_numpy(cands: torch.Tensor) -> np.ndarray:
     return np.ascontiguousarray(a).view(CANDIDATE_DTYPE).reshape(a.shape[0], a.shape[1])
 
 
-def plan_for_workload(wl, n_events: int, n_hits: int, max_hits_per_event: int, device: int = 0) -> Plan:
+def plan_for_workload(wl, n_events: int, n_hits: int, max_hits_per_event: int, device: int = 0, flags: int = 0) -> Plan:
     """Plan of a synth.Workload (grid, threshold, window, K of SURVEY.md Sec. 8(d))."""
     return hough_plan_create(wl.n_theta, wl.n_rho, wl.rho_min, wl.rho_max, wl.coord_max, wl.vote_threshold, wl.assign_window,
                              wl.max_candidates, max(1, n_events), max(0, n_hits), max_hits_per_event,
-                             HOUGH_U16 if wl.count_dtype == "u16" else HOUGH_I32, wl.hit_frac_bits, -1, device)
+                             HOUGH_U16 if wl.count_dtype == "u16" else HOUGH_I32, wl.hit_frac_bits, -1, device, flags)

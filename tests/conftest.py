@@ -8,6 +8,26 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+def pytest_addoption(parser):
+    parser.addoption("--hough-variant", action="store", default="",
+                     help="run the GPU tests against a debug variant of the library (bounds | timers); see DESIGN.md 'GPU gate'")
+    parser.addoption("--gate", action="store_true", default=False,
+                     help="only the small gate cases (<= 8 events each), for the bounds build and compute-sanitizer runs")
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
     config.addinivalue_line("markers", "slow: longer CPU test")
+    config.addinivalue_line("markers", "gate: small GPU case that is safe to run first on an untested build")
+    variant = config.getoption("--hough-variant")
+    if variant:
+        from paper_2511_02742_b200 import build, hough
+        hough.load_library(build.build(variant=variant))
+
+
+def pytest_collection_modifyitems(config, items):
+    if config.getoption("--gate"):
+        skip = pytest.mark.skip(reason="not a gate case")
+        for it in items:
+            if "gate" not in it.keywords:
+                it.add_marker(skip)

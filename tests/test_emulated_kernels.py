@@ -1,0 +1,275 @@
+"""The CUDA kernels of paper_2511_02742_b200/csrc, compiled for the host execution model of tests/emu/cuda_emu.h, against the
+CPU oracle -- element by element, through the same C ABI, on a machine WITHOUT a GPU.
+
+What this proves: the kernels' logic (index arithmetic, list capacities and the hand-over to the general kernel, barrier
+placement against the data flow, per-event resets when one CTA processes many events, results independent of the thread
+schedule) with every shared-memory and "device"-memory access bounds-checked -- the kernels' own -DHOUGH_BOUNDS checks are
+compiled in, shared-window addresses of the PTX accesses are validated, and every allocation ends at an inaccessible page.
+What it does not prove: anything about the hardware (memory model, PTX semantics, timing).  The GPU parity tests
+(tests/test_gpu_parity.py, -m gpu) are the proof of record; these cases mirror them at sizes the model runs in seconds.
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+sys.path.insert(0, os.path.join(os.path.dirname(os.path.abspath(__file__)), "emu"))
+import hough_emu as E  # noqa: E402
+
+from oracle import hough_c as C  # noqa: E402
+from oracle import hough_def as D  # noqa: E402
+from paper_2511_02742_b200 import synth  # noqa: E402
+from test_oracle_pins import edge_cases  # noqa: E402
+from util import mixed_batch, paper_grid_batch, params_of, std_params  # noqa: E402
+
+INT_FIELDS = ("theta_bin", "rho_bin", "votes", "cluster_root", "cluster_nbins", "reserved")
+
+
+@pytest.fixture(autouse=True)
+def default_schedule():
+    E.configure(seed=1, preempt_per_1024=0, smem_window=1024)
+    yield
+    E.configure(seed=1, preempt_per_1024=0, smem_window=1024)
+
+
+def assert_same(g, o, p, status=0):
+    assert g["emu_violations"] == 0, g["emu_first_violation"]
+    assert g["bounds_violations"] == 0, f"index check failed inside a kernel, first at site {g['bounds_site']}"
+    assert g["status"] == status
+    if "acc" in g and o.get("acc") is not None:
+        np.testing.assert_array_equal(g["acc"], o["acc"])
+    if "digest" in g:
+        np.testing.assert_array_equal(g["digest"], o["digest"])
+    np.testing.assert_array_equal(g["n_found"], o["n_found"])
+    for e in range(len(o["n_found"])):
+        k = min(int(o["n_found"][e]), p.max_candidates)
+        ge, oe = g["cands"][e, :k], o["cands"][e, :k]
+        for f in INT_FIELDS:
+            np.testing.assert_array_equal(ge[f], oe[f], err_msg=f"event {e} field {f}")
+        np.testing.assert_allclose(ge["theta"], oe["theta"], rtol=1e-5, atol=0)
+        np.testing.assert_allclose(ge["rho"], oe["rho"], rtol=1e-5, atol=0)
+    np.testing.assert_array_equal(g["labels"], o["labels"])
+
+
+def oracle_run(p, u, v, offsets, want_acc=True):
+    return C.run_batch(u, v, offsets, p, want_digest=True, want_acc=want_acc)
+
+
+def dtype_of(wl):
+    return E.HOUGH_U16 if wl.count_dtype == "u16" else E.HOUGH_I32
+
+
+# ----------------------------------------------------------------------------- BASELINE configs
+@pytest.mark.parametrize("cfg,n_events", [(0, 1), (1, 40), (2, 12), (3, 6)])
+@pytest.mark.parametrize("flags", [0, E.FLAG_SMALL_LISTS, E.FLAG_GENERAL_ONLY], ids=["fast", "small_lists", "general_only"])
+def test_configs_bit_exact(cfg, n_events, flags):
+    wl = synth.workload(cfg)
+    b = synth.generate(wl, 0, n_events)
+    p = params_of(wl)
+    g = E.run(p, b.u, b.v, b.offsets, dtype_of(wl), flags=flags)
+    o = oracle_run(p, b.u, b.v, b.offsets)
+    assert_same(g, o, p)
+    if flags == 0:
+        assert g["info"]["fast_groups"] > 0 and g["deferred"] == 0       # S1-S4 ran in the fast kernel
+    elif flags == E.FLAG_GENERAL_ONLY:
+        assert g["info"]["fast_groups"] == 0 and g["deferred"] == 0
+    elif cfg in (1, 3):
+        assert g["deferred"] > 0                                           # the lists overflowed: handed to the general kernel
+
+
+@pytest.mark.parametrize("seed,preempt", [(2, 0), (3, 8), (4, 64), (5, 512)])
+def test_results_do_not_depend_on_the_schedule(seed, preempt):
+    """Other fiber orders, and a thread switch with probability preempt/1024 at every atomic / cache-bypassing access: lists are
+    filled in another order, union-find races resolve differently -- the outputs may not change."""
+    E.configure(seed=seed, preempt_per_1024=preempt)
+    wl = synth.workload(3)
+    b = synth.generate(wl, 3, 2)
+    p = params_of(wl)
+    for flags in (0, E.FLAG_GENERAL_ONLY):
+        g = E.run(p, b.u, b.v, b.offsets, E.HOUGH_U16, flags=flags, want_vote=False)
+        o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+        assert_same(g, o, p)
+
+
+@pytest.mark.parametrize("window", [0, 1024, 3840, 4096, 8192 + 128])
+def test_shared_window_offset(window):
+    """The vote of the fast kernel folds the tile's shared-window address into the fixed-point offset; the host sized that
+    for a tile below 4096.  Elsewhere the kernel must notice and leave every event to the general kernel."""
+    E.configure(seed=1, smem_window=window)
+    wl = synth.workload(3)
+    b = synth.generate(wl, 0, 2)
+    p = params_of(wl)
+    g = E.run(p, b.u, b.v, b.offsets, E.HOUGH_U16, want_vote=False)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert g["deferred"] == (0 if window < 4096 and window % 256 == 0 else 2)
+
+
+def test_many_events_per_cta():
+    """The model runs the CTAs of a grid one after another, so the first CTA of the persistent grid processes EVERY event:
+    per-event resets (halos, lists, histogram, control block), tile reuse across events, the work counter."""
+    wl = synth.workload(3)
+    b = synth.generate(wl, 0, 24)
+    p = params_of(wl)
+    g = E.run(p, b.u, b.v, b.offsets, E.HOUGH_U16, want_acc=False)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert g["info"]["fast_groups"] > 0 and g["deferred"] == 0
+
+
+def test_mixed_batch_with_deferred_events_interleaved():
+    wl, u, v, offsets, kinds = mixed_batch(1, 400, seed=21)
+    p = params_of(wl)
+    n_big = kinds.count("count>1023")
+    assert n_big >= 3 and kinds.count("empty") >= 5 and kinds.count("invalid") >= 1
+    g = E.run(p, u, v, offsets, max_hpe=2048, want_acc=False)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert g["info"]["fast_groups"] > 0 and g["deferred"] == n_big
+
+
+def test_events_longer_than_the_fast_staging_buffer_are_deferred():
+    wl, u, v, offsets, kinds = mixed_batch(2, 60, seed=23, long_hits=9000)
+    p = params_of(wl)
+    n_long = kinds.count("long")
+    assert n_long >= 1
+    g = E.run(p, u, v, offsets, max_hpe=9000, want_acc=False)
+    assert g["info"]["fast_hits_cap"] < 9000
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert g["deferred"] == n_long + kinds.count("count>1023")
+
+
+@pytest.mark.parametrize("hits_idx", [0, 1, 2, 3])
+@pytest.mark.parametrize("grid_idx", [0, 1, 2, 3])
+def test_config4_cells(hits_idx, grid_idx):
+    wl = synth.workload(4, hits_idx, grid_idx)
+    n_events = {0: 12, 1: 8, 2: 3, 3: 2}[hits_idx]
+    b = synth.generate(wl, 0, n_events)
+    p = params_of(wl)
+    g = E.run(p, b.u, b.v, b.offsets, want_acc=grid_idx < 3)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=grid_idx < 3)
+    assert_same(g, o, p)
+
+
+# ----------------------------------------------------------------------------- adversarial edge set
+@pytest.mark.parametrize("case", edge_cases(), ids=lambda c: c[0])
+def test_edge_set(case):
+    name, p, u, v = case
+    offsets = np.array([0, len(u)], np.int64)
+    for flags in (0, E.FLAG_GENERAL_ONLY):
+        g = E.run(p, u, v, offsets, max_hpe=max(len(u), 1), flags=flags)
+        o = oracle_run(p, u, v, offsets)
+        assert_same(g, o, p)
+
+
+def test_edge_set_as_one_ragged_batch():
+    cases = [c for c in edge_cases() if c[1] == edge_cases()[0][1]]
+    p = cases[0][1]
+    us, vs, offs = [], [], [0]
+    for _, _, u, v in cases:
+        us.append(u); vs.append(v); offs.append(offs[-1] + len(u)); offs.append(offs[-1])
+    u, v, offsets = np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64)
+    g = E.run(p, u, v, offsets)
+    o = oracle_run(p, u, v, offsets)
+    assert_same(g, o, p)
+
+
+def test_strip_seams_dense_mask():
+    rng = np.random.default_rng(12)
+    p = std_params(512, 512, T=3, K=128)
+    u = rng.uniform(-94, 94, 1500).astype(np.float32)
+    v = rng.uniform(-194, 194, 1500).astype(np.float32)
+    offsets = np.array([0, 700, 1500], np.int64)
+    for flags in (0, E.FLAG_GENERAL_ONLY):
+        g = E.run(p, u, v, offsets, flags=flags)
+        o = oracle_run(p, u, v, offsets)
+        assert_same(g, o, p)
+
+
+def test_ties_at_the_kth_vote_count():
+    """More peaks than K with many ties at the K-th count: the tie path of the fast kernel's selection (the count
+    of kept peaks was overwritten while other warps still read it)."""
+    rng = np.random.default_rng(14)
+    p = std_params(256, 256, T=3, K=24)
+    u = rng.uniform(-94, 94, 260).astype(np.float32)
+    v = rng.uniform(-194, 194, 260).astype(np.float32)
+    offsets = np.array([0, 130, 260], np.int64)
+    for seed in (1, 2, 3):
+        E.configure(seed=seed, preempt_per_1024=32)
+        g = E.run(p, u, v, offsets)
+        o = oracle_run(p, u, v, offsets)
+        assert (o["n_found"] > p.max_candidates).all()
+        assert_same(g, o, p)
+        assert g["info"]["fast_groups"] > 0 and g["deferred"] == 0
+
+
+def test_unsafe_hits_near_the_rho_range_edge():
+    rng = np.random.default_rng(11)
+    p = std_params(256, 256, T=4, K=64)
+    u = rng.uniform(-256, 256, 600).astype(np.float32)
+    v = rng.uniform(-256, 256, 600).astype(np.float32)
+    offsets = np.array([0, 100, 100, 350, 600], np.int64)
+    g = E.run(p, u, v, offsets)
+    o = oracle_run(p, u, v, offsets)
+    assert_same(g, o, p)
+    assert g["acc"].sum() < 600 * 256
+
+
+def test_large_K_and_overflowing_peak_list():
+    rng = np.random.default_rng(13)
+    p = std_params(512, 512, T=1, K=4096)
+    u = rng.uniform(-94, 94, 300).astype(np.float32)
+    v = rng.uniform(-194, 194, 300).astype(np.float32)
+    offsets = np.array([0, 300], np.int64)
+    g = E.run(p, u, v, offsets, want_acc=False)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert o["n_found"][0] > 4096
+    assert_same(g, o, p)
+
+
+def test_many_hits_per_event_is_staged_in_chunks():
+    wl = synth.workload(4, 3, 1)
+    b = synth.generate(wl, 0, 2)
+    p = params_of(wl, max_candidates=16)
+    g = E.run(p, b.u, b.v, b.offsets, flags=E.FLAG_GENERAL_ONLY)
+    o = oracle_run(p, b.u, b.v, b.offsets)
+    assert_same(g, o, p)
+
+
+def test_status_word_flags_long_events():
+    p = std_params(64, 64, T=3, K=8)
+    rng = np.random.default_rng(2)
+    u = rng.uniform(-100, 100, 300).astype(np.float32)
+    v = rng.uniform(-100, 100, 300).astype(np.float32)
+    offsets = np.array([0, 50, 250, 300], np.int64)
+    g = E.run(p, u, v, offsets, max_hpe=100, want_vote=False)
+    assert g["emu_violations"] == 0 and g["bounds_violations"] == 0
+    assert g["status"] & 1
+    assert g["n_found"][1] == 0 and (g["labels"][50:250] == -1).all()
+    o = C.run_batch(u[:50], v[:50], np.array([0, 50], np.int64), p)
+    np.testing.assert_array_equal(g["labels"][:50], o["labels"])
+
+
+def test_paper_grid_180x1000_multi_event():
+    p, u, v, offsets = paper_grid_batch(24)
+    g = E.run(p, u, v, offsets, want_acc=False)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert_same(g, o, p)
+
+
+@pytest.mark.parametrize("n_chunks,n_events", [(0, 12), (3, 40), (7, 40), (32, 40)])
+def test_run_host_chunked(n_chunks, n_events):
+    wl = synth.workload(1)
+    b = synth.generate(wl, 0, n_events)
+    p = params_of(wl)
+    offsets = np.concatenate([b.offsets[:n_events // 2], np.repeat(b.offsets[n_events // 2], 3), b.offsets[n_events // 2:]])
+    g = E.run_host(p, b.u, b.v, offsets, n_chunks, repeat=2)
+    assert g["emu_violations"] == 0, g["emu_first_violation"]
+    o = C.run_batch(b.u, b.v, offsets, p)
+    np.testing.assert_array_equal(g["n_found"], o["n_found"])
+    np.testing.assert_array_equal(g["labels"], o["labels"])
+    for e in range(len(offsets) - 1):
+        k = min(int(o["n_found"][e]), p.max_candidates)
+        assert g["cands"][e, :k].tobytes() == o["cands"][e, :k].tobytes()

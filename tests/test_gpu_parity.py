@@ -10,37 +10,43 @@ from oracle import hough_def as D
 from paper_2511_02742_b200 import hough as H
 from paper_2511_02742_b200 import synth
 from test_oracle_pins import edge_cases
-from util import params_of, std_params
+from util import mixed_batch, paper_grid_batch, params_of, std_params
 
 pytestmark = pytest.mark.gpu
 
 INT_FIELDS = ("theta_bin", "rho_bin", "votes", "cluster_root", "cluster_nbins", "reserved")
 
 
-def make_plan(p: D.Params, n_events, n_hits, max_hpe, count_dtype=H.HOUGH_I32):
+def make_plan(p: D.Params, n_events, n_hits, max_hpe, count_dtype=H.HOUGH_I32, flags=0):
     return H.hough_plan_create(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.vote_threshold, p.assign_window,
                                p.max_candidates, max(1, n_events), max(0, n_hits), max_hpe, count_dtype,
-                               p.hit_frac_bits, p.acc_frac_bits, 0)
+                               p.hit_frac_bits, p.acc_frac_bits, 0, flags)
 
 
-def gpu_run(p: D.Params, u, v, offsets, count_dtype=H.HOUGH_I32, want_acc=True, max_hpe=None):
-    """Whole CUDA path on one batch; returns numpy results shaped like oracle.hough_c.run_batch."""
+def gpu_run(p: D.Params, u, v, offsets, count_dtype=H.HOUGH_I32, want_acc=True, max_hpe=None, flags=0, want_vote=True):
+    """Whole CUDA path on one batch; returns numpy results shaped like oracle.hough_c.run_batch, plus which kernel did the
+    work: info["fast_groups"] (0 = the plan has no fast kernel) and "deferred" (events the fast kernel handed over)."""
     E = len(offsets) - 1
     hpe = int(np.diff(offsets).max()) if E > 0 and len(u) else 0
-    plan = make_plan(p, E, len(u), max(hpe, 1) if max_hpe is None else max_hpe, count_dtype)
+    plan = make_plan(p, E, len(u), max(hpe, 1) if max_hpe is None else max_hpe, count_dtype, flags)
     du = torch.from_numpy(np.ascontiguousarray(u, np.float32)).cuda()
     dv = torch.from_numpy(np.ascontiguousarray(v, np.float32)).cuda()
     do = torch.from_numpy(np.ascontiguousarray(offsets, np.int64)).cuda()
     out = {}
-    acc, dig = H.hough_vote(plan, du, dv, do, want_acc=want_acc, want_digest=True)
+    acc = dig = None
+    if want_vote:
+        acc, dig = H.hough_vote(plan, du, dv, do, want_acc=want_acc, want_digest=True)
     cands, n_found = H.hough_find_clusters(plan, du, dv, do)
     labels = H.hough_assign_hits(plan, du, dv, do, cands, n_found)
     torch.cuda.synchronize()
+    dbg = H.hough_plan_debug_counters(plan)
+    out["deferred"], out["bounds_violations"], out["bounds_site"] = int(dbg[15]), int(dbg[14]), int(dbg[13])
     out["status"] = H.hough_plan_status(plan)
     if acc is not None:
         a = acc.cpu().numpy()
         out["acc"] = a.view(np.uint16).astype(np.int32) if a.dtype == np.int16 else a
-    out["digest"] = dig.cpu().numpy().view(np.uint64)
+    if dig is not None:
+        out["digest"] = dig.cpu().numpy().view(np.uint64)
     out["cands"] = H.candidates_to_numpy(cands)
     out["n_found"] = n_found.cpu().numpy()
     out["labels"] = labels.cpu().numpy()
@@ -49,11 +55,13 @@ def gpu_run(p: D.Params, u, v, offsets, count_dtype=H.HOUGH_I32, want_acc=True, 
     return out
 
 
-def assert_same(g, o, p: D.Params, check_acc=True):
-    assert g["status"] == 0
+def assert_same(g, o, p: D.Params, check_acc=True, status=0):
+    assert g["bounds_violations"] == 0, f"index check failed inside a kernel, first at site {g['bounds_site']}"
+    assert g["status"] == status
     if check_acc and "acc" in g:
         np.testing.assert_array_equal(g["acc"], o["acc"])
-    np.testing.assert_array_equal(g["digest"], o["digest"])
+    if "digest" in g:
+        np.testing.assert_array_equal(g["digest"], o["digest"])
     np.testing.assert_array_equal(g["n_found"], o["n_found"])
     for e in range(len(o["n_found"])):
         k = min(int(o["n_found"][e]), p.max_candidates)
@@ -65,8 +73,17 @@ def assert_same(g, o, p: D.Params, check_acc=True):
     np.testing.assert_array_equal(g["labels"], o["labels"])
 
 
-def oracle_run(p, u, v, offsets):
-    return C.run_batch(u, v, offsets, p, want_digest=True, want_acc=True)
+def oracle_run(p, u, v, offsets, want_acc=True):
+    return C.run_batch(u, v, offsets, p, want_digest=True, want_acc=want_acc)
+
+
+def assert_path(g, fast: bool, deferred=None):
+    """Which kernel produced the result: the plan has (no) fast kernel; `deferred` = 0, an exact count, or ">0"."""
+    assert (g["info"]["fast_groups"] > 0) == fast, g["info"]
+    if deferred == ">0":
+        assert g["deferred"] > 0
+    elif deferred is not None:
+        assert g["deferred"] == deferred, g["deferred"]
 
 
 # ----------------------------------------------------------------------------- tables first (DESIGN.md: libm check)
@@ -83,6 +100,21 @@ def test_tables_and_constants_equal_oracle(grid):
 
 
 # ----------------------------------------------------------------------------- BASELINE configs at oracle-sized samples
+@pytest.mark.gate
+@pytest.mark.parametrize("cfg,n_events", [(0, 1), (1, 8), (2, 4), (3, 3)])
+def test_gate_configs_small(cfg, n_events):
+    """The first thing an untested build runs: at most 8 events per config."""
+    wl = synth.workload(cfg)
+    b = synth.generate(wl, 0, n_events)
+    p = params_of(wl)
+    dt = H.HOUGH_U16 if wl.count_dtype == "u16" else H.HOUGH_I32
+    for flags, fast, deferred in ((0, True, 0), (H.HOUGH_FLAG_SMALL_LISTS, True, None), (H.HOUGH_FLAG_GENERAL_ONLY, False, 0)):
+        g = gpu_run(p, b.u, b.v, b.offsets, dt, flags=flags)
+        o = oracle_run(p, b.u, b.v, b.offsets)
+        assert_same(g, o, p)
+        assert_path(g, fast, deferred)
+
+
 @pytest.mark.parametrize("cfg,n_events", [(0, 1), (1, 96), (2, 40), (3, 12)])
 def test_configs_bit_exact(cfg, n_events):
     wl = synth.workload(cfg)
@@ -92,20 +124,101 @@ def test_configs_bit_exact(cfg, n_events):
     g = gpu_run(p, b.u, b.v, b.offsets, dt)
     o = oracle_run(p, b.u, b.v, b.offsets)
     assert_same(g, o, p)
+    assert_path(g, fast=True, deferred=0)              # S1-S4 of these events ran in the fast kernel
     assert g["acc"].sum() == b.n_hits * wl.n_theta     # P4: every generator hit votes once per theta row
 
 
-@pytest.mark.parametrize("hits_idx,grid_idx,n_events", [(0, 0, 6), (0, 3, 3), (1, 1, 6), (2, 2, 4), (3, 0, 3), (3, 3, 2), (2, 3, 2), (3, 1, 2)])
-def test_config4_cells_bit_exact(hits_idx, grid_idx, n_events):
-    wl = synth.workload(4, hits_idx, grid_idx)
+@pytest.mark.parametrize("cfg,n_events", [(1, 2400), (3, 640)])
+def test_many_events_per_cta_fast_kernel(cfg, n_events):
+    """More events than 4 x the persistent CTAs: every CTA processes several events back to back (per-event reset of halos,
+    lists and histogram, tile reuse, work counter).  Digests prove the accumulators, records and labels the rest."""
+    wl = synth.workload(cfg)
     b = synth.generate(wl, 0, n_events)
     p = params_of(wl)
-    g = gpu_run(p, b.u, b.v, b.offsets)
-    o = oracle_run(p, b.u, b.v, b.offsets)
+    dt = H.HOUGH_U16 if wl.count_dtype == "u16" else H.HOUGH_I32
+    g = gpu_run(p, b.u, b.v, b.offsets, dt, want_acc=False)
+    assert n_events >= 4 * g["info"]["fast_ctas"]
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert_path(g, fast=True, deferred=0)
+
+
+def test_mixed_batch_with_deferred_events_interleaved():
+    wl, u, v, offsets, kinds = mixed_batch(1, 1500, seed=21)
+    p = params_of(wl)
+    n_big = kinds.count("count>1023")
+    assert n_big >= 10 and kinds.count("empty") >= 20
+    g = gpu_run(p, u, v, offsets, want_acc=False, max_hpe=2048)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert_path(g, fast=True, deferred=n_big)          # exactly the events with a count above 1023 were handed over
+    big = kinds.index("count>1023")
+    assert o["cands"][big, 0]["votes"] == 1100
+
+
+def test_events_longer_than_the_fast_staging_buffer_are_deferred():
+    wl, u, v, offsets, kinds = mixed_batch(2, 300, seed=22, long_hits=9000)
+    p = params_of(wl)
+    n_long = kinds.count("long")
+    assert n_long >= 2
+    g = gpu_run(p, u, v, offsets, want_acc=False, max_hpe=9000)
+    assert g["info"]["fast_hits_cap"] < 9000
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert_path(g, fast=True, deferred=n_long + kinds.count("count>1023"))
+
+
+@pytest.mark.parametrize("cfg,n_events", [(1, 400), (3, 160)])
+def test_small_lists_force_the_hand_over(cfg, n_events):
+    """HOUGH_FLAG_SMALL_LISTS: ordinary events overflow the fast kernel's lists mid-way (strip list, on list, peak list) and
+    are recomputed by the general kernel; results stay identical."""
+    wl = synth.workload(cfg)
+    b = synth.generate(wl, 0, n_events)
+    p = params_of(wl)
+    dt = H.HOUGH_U16 if wl.count_dtype == "u16" else H.HOUGH_I32
+    g = gpu_run(p, b.u, b.v, b.offsets, dt, want_acc=False, flags=H.HOUGH_FLAG_SMALL_LISTS)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert_path(g, fast=True, deferred=">0")
+
+
+@pytest.mark.parametrize("cfg,n_events", [(1, 700), (3, 40)])
+def test_general_kernel_alone(cfg, n_events):
+    wl = synth.workload(cfg)
+    b = synth.generate(wl, 0, n_events)
+    p = params_of(wl)
+    dt = H.HOUGH_U16 if wl.count_dtype == "u16" else H.HOUGH_I32
+    g = gpu_run(p, b.u, b.v, b.offsets, dt, want_acc=False, flags=H.HOUGH_FLAG_GENERAL_ONLY)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert_path(g, fast=False, deferred=0)
+
+
+def test_paper_grid_180x1000_multi_event():
+    """The paper's own CPU grid (180 theta bins over 0-180 deg, 1000 rho bins over -500...500), 40 planes
+    (L72 "40 vanes"), a batch of events."""
+    p, u, v, offsets = paper_grid_batch(200)
+    g = gpu_run(p, u, v, offsets, want_acc=False)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert (o["n_found"] >= 1).all()
+
+
+@pytest.mark.parametrize("hits_idx", [0, 1, 2, 3])
+@pytest.mark.parametrize("grid_idx", [0, 1, 2, 3])
+def test_config4_cells_bit_exact(hits_idx, grid_idx):
+    """All 16 cells of the roofline sweep (hits/event x grid), enough events that CTAs of the fast kernel take several."""
+    wl = synth.workload(4, hits_idx, grid_idx)
+    n_events = {0: 320, 1: 160, 2: 24, 3: 6}[hits_idx] if grid_idx < 3 else {0: 40, 1: 24, 2: 8, 3: 3}[hits_idx]
+    b = synth.generate(wl, 0, n_events)
+    p = params_of(wl)
+    g = gpu_run(p, b.u, b.v, b.offsets, want_acc=(n_events <= 24 and grid_idx < 3))
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=(n_events <= 24 and grid_idx < 3))
     assert_same(g, o, p)
 
 
 # ----------------------------------------------------------------------------- adversarial edge set
+@pytest.mark.gate
 @pytest.mark.parametrize("case", edge_cases(), ids=lambda c: c[0])
 def test_edge_set(case):
     name, p, u, v = case
@@ -115,6 +228,7 @@ def test_edge_set(case):
     assert_same(g, o, p)
 
 
+@pytest.mark.gate
 def test_edge_set_as_one_ragged_batch():
     """Same grid cases concatenated into one batch with empty events in between (ragged offsets, unaligned starts)."""
     cases = [c for c in edge_cases() if c[1] == edge_cases()[0][1]]
@@ -234,26 +348,35 @@ def test_status_word_flags_long_events_and_bad_offsets():
     np.testing.assert_array_equal(g["labels"][:50], o["labels"])
 
 
-def test_run_host_equals_device_calls():
+@pytest.mark.parametrize("n_chunks,n_events", [(0, 32), (1, 32), (3, 500), (7, 500), (32, 40)])
+def test_run_host_chunked_equals_oracle(n_chunks, n_events):
+    """hough_run_host / hough_run_host_chunked: the three-stream chunk pipeline (upload, compute, download), called twice on
+    one plan; chunk boundaries fall inside the batch, with empty events around them."""
     wl = synth.workload(1)
-    b = synth.generate(wl, 0, 32)
+    b = synth.generate(wl, 0, n_events)
     p = params_of(wl)
-    plan = make_plan(p, 32, b.n_hits, int(np.diff(b.offsets).max()))
-    cands = np.zeros((32, p.max_candidates, 8), np.int32)
-    n_found = np.zeros(32, np.int32)
-    labels = np.zeros(b.n_hits, np.int32)
-    H.hough_run_host(plan, b.u, b.v, b.offsets, cands, n_found, labels)
-    fast = H.hough_plan_query(plan)[0]["fast_groups"] > 0          # fast kernel + general kernel on its deferred list
-    assert H.hough_plan_launch_count(plan) == (3 if fast else 2)
+    offsets = np.concatenate([b.offsets[:n_events // 2], np.repeat(b.offsets[n_events // 2], 3), b.offsets[n_events // 2:]])  # + 3 empty events
+    E = len(offsets) - 1
+    plan = make_plan(p, E, b.n_hits, int(np.diff(offsets).max()))
+    o = C.run_batch(b.u, b.v, offsets, p)
+    for rep in range(2):
+        cands = np.zeros((E, p.max_candidates, 8), np.int32)
+        n_found = np.full(E, -7, np.int32)
+        labels = np.full(b.n_hits, -7, np.int32)
+        before = H.hough_plan_launch_count(plan)
+        H.hough_run_host(plan, b.u, b.v, offsets, cands, n_found, labels, n_chunks=n_chunks)
+        chunks_run = (H.hough_plan_launch_count(plan) - before) // 3    # fast + general-on-deferred + assign per chunk
+        want = 1 if n_chunks == 0 else min(n_chunks, E)
+        assert chunks_run == want if want <= 7 else 1 <= chunks_run <= want     # (a chunk without events launches nothing)
+        np.testing.assert_array_equal(n_found, o["n_found"])
+        np.testing.assert_array_equal(labels, o["labels"])
+        gc = cands.view(H.CANDIDATE_DTYPE).reshape(E, p.max_candidates)
+        for e in range(E):
+            k = min(int(n_found[e]), p.max_candidates)
+            for f in INT_FIELDS:
+                np.testing.assert_array_equal(gc[e, :k][f], o["cands"][e, :k][f])
+    assert H.hough_plan_status(plan) == 0
     H.hough_plan_destroy(plan)
-    o = C.run_batch(b.u, b.v, b.offsets, p)
-    np.testing.assert_array_equal(n_found, o["n_found"])
-    np.testing.assert_array_equal(labels, o["labels"])
-    gc = cands.view(H.CANDIDATE_DTYPE).reshape(32, p.max_candidates)
-    for e in range(32):
-        k = min(int(n_found[e]), p.max_candidates)
-        for f in INT_FIELDS:
-            np.testing.assert_array_equal(gc[e, :k][f], o["cands"][e, :k][f])
 
 
 def test_bad_arguments_are_rejected_not_crashed():

@@ -4,6 +4,7 @@ import os
 import numpy as np
 
 from oracle import hough_def as D
+from paper_2511_02742_b200 import synth
 
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 
@@ -46,3 +47,49 @@ def cands_as_tuples(cands):
         else:
             out.append((int(c["theta_bin"]), int(c["rho_bin"]), int(c["votes"]), int(c["cluster_root"]), int(c["cluster_nbins"])))
     return out
+
+
+def mixed_batch(cfg, n_events, seed, long_hits=0):
+    """Generator events with special ones interleaved: empty events, an event whose hits all coincide 1100 times (a bin count
+    above 1023: the fast kernel must hand it over), all-invalid events, and optionally one event of `long_hits` hits."""
+    wl = synth.workload(cfg)
+    b = synth.generate(wl, 0, n_events)
+    rng = np.random.default_rng(seed)
+    us, vs, offs, kinds = [], [], [0], []
+    for e in range(n_events):
+        a, z = int(b.offsets[e]), int(b.offsets[e + 1])
+        roll = rng.random()
+        if roll < 0.05:
+            uu, vv, kind = np.zeros(0, np.float32), np.zeros(0, np.float32), "empty"
+        elif roll < 0.08:
+            uu, vv, kind = np.full(1100, 7.25, np.float32), np.full(1100, -3.5, np.float32), "count>1023"
+        elif roll < 0.10:
+            uu, vv, kind = np.full(17, np.nan, np.float32), np.full(17, 1.0, np.float32), "invalid"
+        elif long_hits and roll < 0.12:
+            uu = rng.uniform(-94, 94, long_hits).astype(np.float32)
+            vv = rng.uniform(-194, 194, long_hits).astype(np.float32)
+            kind = "long"
+        else:
+            uu, vv, kind = b.u[a:z], b.v[a:z], "plain"
+        us.append(uu); vs.append(vv); offs.append(offs[-1] + len(uu)); kinds.append(kind)
+    return wl, np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64), kinds
+
+
+def paper_grid_batch(n_events, seed=31):
+    """Events on the paper's own CPU grid (180 theta bins over 0-180 deg, 1000 rho bins over -500...500) with
+    40 detector planes (L72: 40 vanes): 1-8 straight tracks plus up to 200 noise hits per event.  -> (params, u, v, offsets)"""
+    rng = np.random.default_rng(seed)
+    p = D.Params(180, 1000, -500.0, 500.0, 360.0, 20, 1.0, 64)
+    us, vs, offs = [], [], [0]
+    planes = np.linspace(-195.0, 195.0, 40)
+    for e in range(n_events):
+        nt = int(rng.integers(1, 9))
+        uu = [np.tile(planes, nt)]
+        m, c = rng.uniform(-1, 1, nt), rng.uniform(-100, 100, nt)
+        vv = [(m[:, None] * planes[None, :] + c[:, None] + rng.normal(0, 0.1, (nt, 40))).ravel()]
+        nn = int(rng.integers(0, 200))
+        uu.append(rng.uniform(-195, 195, nn)); vv.append(rng.uniform(-300, 300, nn))
+        uu, vv = np.concatenate(uu).astype(np.float32), np.concatenate(vv).astype(np.float32)
+        pm = rng.permutation(len(uu))
+        us.append(uu[pm]); vs.append(vv[pm]); offs.append(offs[-1] + len(uu))
+    return p, np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64)
