@@ -136,6 +136,80 @@ int hough_assign_hits(hough_plan_t* plan, const float* d_u, const float* d_v, co
                       int32_t n_events, const hough_candidate_t* d_cands, const int32_t* d_n_found,
                       int32_t* d_labels, void* stream);
 
+/* ---- stages around the core (O9-O13) ---- */
+
+/* Detector planes (vanes) along u, for the "found" criterion of PAPER.md L136 (Sec. 7: "a track is regarded as found if its
+ * hits are reconstructed and clustered in continuous five vanes"): plane k sits at u = plane_origin + k plane_pitch; a hit
+ * belongs to its nearest plane, floor((u - origin) / pitch + 1/2), evaluated on the fixed-point coordinate. */
+typedef struct {
+    double plane_origin, plane_pitch;   /* pitch > 0; pitch * 2^H must round to >= 1                               */
+    int32_t n_planes;                   /* 1 .. 64                                                                  */
+    int32_t min_run;                    /* consecutive planes with a hit that make a track "found"; <= 0 -> 5       */
+    int32_t wrap;                       /* != 0: the planes form a ring (plane n_planes - 1 is next to plane 0)     */
+    int32_t reserved;                   /* 0                                                                        */
+} hough_plane_geometry_t;
+
+enum { HOUGH_FIT_FOUND = 1, HOUGH_FIT_DEGENERATE = 2 };
+
+/* Refit of one kept candidate from the hits labelled with its slot.  32 bytes, little endian. */
+typedef struct {
+    int32_t n_hits;                     /* hits assigned to the slot                                                */
+    int32_t max_run;                    /* longest run of consecutive planes that hold such a hit                   */
+    uint64_t plane_mask;                /* bit k set iff plane k holds one                                          */
+    float slope, intercept;             /* least-squares line v = slope u + intercept through the fixed-point hits  */
+    int32_t flags;                      /* HOUGH_FIT_FOUND: max_run >= min_run; HOUGH_FIT_DEGENERATE: fewer than two
+                                           hits, or all hits at one u (no slope; slope = intercept = 0)             */
+    int32_t reserved;                   /* 0                                                                        */
+} hough_fit_t;
+
+/* Straight-line refit of every kept candidate (the stand-in for the paper's seed fit, "the corresponding
+ * RecoHits lying along it are used as seeds", L112-114) and the found criterion (L136).  The sums are exact 64-bit integers
+ * of the fixed-point coordinates, so the result does not depend on the order of the hits.
+ *   d_n_found, d_labels   as written by hough_find_clusters / hough_assign_hits for the same events
+ *   d_fits                [n_events][K]; event e gets min(n_found[e], K) records, the rest of its row is left untouched
+ * HOUGH_ERANGE if the plan's coord_max * 2^H exceeds 2^15 or its max_hits_per_event exceeds 65535 (the sums would overflow). */
+int hough_refit_tracks(hough_plan_t* plan, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events,
+                       const int32_t* d_n_found, const int32_t* d_labels, const hough_plane_geometry_t* geometry,
+                       hough_fit_t* d_fits, void* stream);
+
+/* Front end: RecoHits (x, y, z, t) of a batch of fills -> one event per time window, in the (phi, z) plane.
+ * "the reconstructed hit points are divided into overlapping time windows of 10 ns, with a sliding step of
+ * 5 ns.  Within each time window, the spatial coordinates (x, y, z) of the hits are transformed into the (phi, z) space".
+ * Window w of every fill covers t0 + w step <= t < t0 + w step + width (times rounded to 2^-8 ns, ties to even).  phi =
+ * atan2(y, x) in degrees, [-180, 180], by a 20-step integer CORDIC on x, y rounded to 2^-6 mm with the angle table
+ * llround(atan(2^-i) 180 / pi 2^16): identical bits on every machine, within 4e-4 degree of atan2 for radii >= 1 mm. */
+typedef struct hough_frontend hough_frontend_t;
+typedef struct {
+    double t0, window_width, window_step;   /* ns; width, step > 0 (PAPER.md: 10 and 5)                            */
+    int32_t windows_per_fill;               /* >= 1; event index of window w of fill f = f * windows_per_fill + w   */
+    double xy_max;                          /* a hit is valid iff finite, |x|, |y| <= xy_max (<= 512), (x, y) != 0  */
+    int32_t max_fills;                      /* capacity: fills per call                                             */
+    int64_t max_hits;                       /* capacity: input hits per call                                        */
+    int32_t device;
+    int32_t reserved;                       /* 0                                                                    */
+} hough_frontend_desc_t;
+
+enum { HOUGH_STATUS_OUTPUT_TRUNCATED = 8 };   /* front-end status bit: the output arrays were too small             */
+
+int hough_frontend_create(const hough_frontend_desc_t* desc, hough_frontend_t** out);
+int hough_frontend_destroy(hough_frontend_t* fe);
+
+/* Enqueues the slicing on `stream` (no host synchronisation).
+ *   d_x, d_y, d_z, d_t   [n_hits] fp32 RecoHits (mm, ns), structure of arrays
+ *   d_fill_offsets       [n_fills + 1] int64, non-decreasing, fill f owns hits [fill_offsets[f], fill_offsets[f+1])
+ *   d_u, d_v             [capacity] fp32 out: phi (degrees) and z of the windows' hits, window after window; inside a window
+ *                        the hits keep their input order
+ *   d_src                [capacity] int32 out: index of the input hit each output hit came from
+ *   d_offsets            [n_fills * windows_per_fill + 1] int64 out: event offsets for hough_vote / hough_find_clusters / ...
+ *                        always complete, even if the hits did not fit (then HOUGH_STATUS_OUTPUT_TRUNCATED is set and
+ *                        d_offsets[last] tells the capacity that is needed; at most ceil(width / step) * n_hits) */
+int hough_frontend_slice(hough_frontend_t* fe, const float* d_x, const float* d_y, const float* d_z, const float* d_t,
+                         const int64_t* d_fill_offsets, int32_t n_fills, int64_t n_hits, float* d_u, float* d_v,
+                         int32_t* d_src, int64_t* d_offsets, int64_t capacity, void* stream);
+
+/* Reads and clears the front end's device status word.  Synchronises `stream`. */
+int hough_frontend_status(hough_frontend_t* fe, int32_t* out, void* stream);
+
 /* ---- helpers beyond the five ---- */
 
 /* hough_find_clusters + hough_assign_hits on HOST buffers (pinned memory makes the copies asynchronous): the batch is cut

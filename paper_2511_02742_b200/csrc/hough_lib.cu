@@ -4,6 +4,7 @@
 #include "../../include/hough.h"
 #include "hough_kernels.cuh"
 #include "hough_fast.cuh"
+#include "hough_track.cuh"
 
 #include <math.h>
 #include <stdio.h>
@@ -18,6 +19,8 @@ using hough::DevParams;
 
 static_assert(sizeof(hough_candidate_t) == 32, "record layout");
 static_assert(sizeof(Candidate) == sizeof(hough_candidate_t), "device record mirrors the ABI record");
+static_assert(sizeof(hough_fit_t) == 32 && sizeof(hough::Fit) == sizeof(hough_fit_t), "fit record layout");
+static_assert(sizeof(hough::FitAcc) == 48, "per-candidate accumulator");
 
 // kernel launch: the <<< >>> syntax, or the host model of tests/emu when the sources are compiled for the CPU tests
 #ifdef HOUGH_EMU
@@ -752,6 +755,149 @@ int hough_measure_smem_atomic_peak(int32_t device, double millis, double* ops_pe
     if (sm_clock_mhz) *sm_clock_mhz = avg / (ms * 1e-3) / 1e6;
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(d_cyc); cudaFree(d_sink);
+    return HOUGH_OK;
+}
+
+// ---------------------------------------------------------------- back end: refit + found criterion (hough_track.cuh)
+
+int hough_refit_tracks(hough_plan_t* p, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events,
+                       const int32_t* d_n_found, const int32_t* d_labels, const hough_plane_geometry_t* g, hough_fit_t* d_fits,
+                       void* stream)
+{
+    int rc = check_common(p, d_u, d_v, d_offsets, n_events);
+    if (rc) return rc;
+    if (!d_n_found || !g || !d_fits || ((uintptr_t)d_fits & 15)) return HOUGH_EINVAL;
+    if (g->n_planes < 1 || g->n_planes > 64 || !(g->plane_pitch > 0) || !isfinite(g->plane_pitch) || !isfinite(g->plane_origin)) return HOUGH_EINVAL;
+    const int H = p->desc.hit_frac_bits;
+    // exact 64-bit sums need |u_q|, |v_q| <= 2^15 and fewer than 2^16 hits per event
+    if (floor(p->desc.coord_max * ldexp(1.0, H)) > 32768.0 || p->desc.max_hits_per_event > 65535) return HOUGH_ERANGE;
+    const double oq_d = g->plane_origin * ldexp(1.0, H), pq_d = g->plane_pitch * ldexp(1.0, H);
+    if (fabs(oq_d) > 1073741823.0 || pq_d > 1073741823.0 || llround(pq_d) < 1) return HOUGH_ERANGE;
+    if (n_events == 0) return HOUGH_OK;
+    if (!d_labels) return HOUGH_EINVAL;
+    hough::PlaneParams G;
+    G.oq = (int)llround(oq_d); G.pq = (int)llround(pq_d);
+    G.n_planes = g->n_planes; G.min_run = g->min_run > 0 ? g->min_run : 5; G.wrap = g->wrap != 0;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(p->desc.device));
+    const size_t smem = (size_t)p->P.K * sizeof(hough::FitAcc);
+    if (smem > 48 * 1024) HCK(cudaFuncSetAttribute(hough::hough_refit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int grid = n_events < p->assign_ctas ? n_events : p->assign_ctas;
+    HOUGH_LAUNCH(hough::hough_refit_kernel, grid, 256, smem, st, p->P, G, d_u, d_v, reinterpret_cast<const long long*>(d_offsets), n_events,
+                 d_n_found, d_labels, reinterpret_cast<hough::Fit*>(d_fits));
+    HCK(cudaGetLastError());
+    p->launches += 1;
+    return HOUGH_OK;
+}
+
+// ---------------------------------------------------------------- front end: time slicing + phi (hough_track.cuh)
+
+struct hough_frontend {
+    hough_frontend_desc_t desc;
+    hough::FrontParams FP;
+    int n_sm;
+    void* d_scratch;
+};
+
+int hough_frontend_create(const hough_frontend_desc_t* d, hough_frontend_t** out)
+{
+    if (!d || !out) return HOUGH_EINVAL;
+    if (!(d->window_width > 0) || !(d->window_step > 0) || !isfinite(d->t0) || !isfinite(d->window_width) || !isfinite(d->window_step)) return HOUGH_EINVAL;
+    if (d->windows_per_fill < 1 || d->max_fills < 1 || d->max_hits < 0 || d->device < 0 || d->reserved != 0) return HOUGH_EINVAL;
+    if (!(d->xy_max > 0) || !isfinite(d->xy_max)) return HOUGH_EINVAL;
+    if (d->xy_max > 512.0) return HOUGH_ERANGE;  // |x_q| <= 2^15 keeps the CORDIC state inside int32
+    const double st = ldexp(1.0, hough::kTimeFracBits);
+    const double t0q = d->t0 * st, sq = d->window_step * st, wq = d->window_width * st;
+    if (fabs(t0q) > 1073741823.0 || sq > 1073741823.0 || wq > 1073741823.0 || llround(sq) < 1 || llround(wq) < 1) return HOUGH_ERANGE;
+    if ((double)d->max_fills * d->windows_per_fill > 2147483647.0 || d->max_hits > 2147483647ll) return HOUGH_ERANGE;  // int32 src indices
+    int dev_count = 0;
+    cudaError_t ce = cudaGetDeviceCount(&dev_count);
+    if (ce != cudaSuccess) return cuda_fail(ce, "cudaGetDeviceCount");
+    if (d->device >= dev_count) return HOUGH_EINVAL;
+    cudaDeviceProp prop;
+    HCK(cudaSetDevice(d->device));
+    HCK(cudaGetDeviceProperties(&prop, d->device));
+    hough_frontend* fe = new (std::nothrow) hough_frontend();
+    if (!fe) return HOUGH_ENOMEM;
+    fe->desc = *d;
+    fe->n_sm = prop.multiProcessorCount;
+    hough::FrontParams& FP = fe->FP;
+    memset(&FP, 0, sizeof FP);
+    FP.t0q = (int)llround(t0q); FP.stepq = (int)llround(sq); FP.widthq = (int)llround(wq);
+    FP.windows_per_fill = d->windows_per_fill;
+    FP.xy_max = (float)d->xy_max;
+    if ((double)FP.xy_max > d->xy_max) FP.xy_max = nextafterf(FP.xy_max, 0.0f);  // the fp32 compare must equal the double one
+    for (int i = 0; i < hough::kCordicIters; ++i)
+        FP.atan_q[i] = (int)llround(atan(ldexp(1.0, -i)) * (180.0 / 3.14159265358979323846) * ldexp(1.0, hough::kPhiFracBits));
+    const size_t nh = (size_t)(d->max_hits > 0 ? d->max_hits : 1), nw = (size_t)d->max_fills * d->windows_per_fill;
+    const size_t b_phi = align_up(nh * 4, 256), b_wr = align_up(nh * 8, 256), b_cnt = align_up(nw * 4, 256), b_cur = align_up(nw * 8, 256);
+    ce = cudaMalloc(&fe->d_scratch, b_phi + b_wr + b_cnt + b_cur + 256);
+    if (ce != cudaSuccess) { delete fe; (void)cudaGetLastError(); return ce == cudaErrorMemoryAllocation ? HOUGH_ENOMEM : cuda_fail(ce, "cudaMalloc"); }
+    unsigned char* b = static_cast<unsigned char*>(fe->d_scratch);
+    FP.wrange = reinterpret_cast<int2*>(b);           b += b_wr;
+    FP.cursor = reinterpret_cast<long long*>(b);      b += b_cur;
+    FP.phi = reinterpret_cast<float*>(b);             b += b_phi;
+    FP.counts = reinterpret_cast<int*>(b);            b += b_cnt;
+    FP.status = reinterpret_cast<int*>(b);
+    ce = cudaMemset(FP.status, 0, 256);
+    if (ce != cudaSuccess) { cudaFree(fe->d_scratch); delete fe; return cuda_fail(ce, "cudaMemset"); }
+    *out = fe;
+    return HOUGH_OK;
+}
+
+int hough_frontend_destroy(hough_frontend_t* fe)
+{
+    if (!fe) return HOUGH_OK;
+    (void)cudaSetDevice(fe->desc.device);
+    (void)cudaDeviceSynchronize();
+    cudaFree(fe->d_scratch);
+    (void)cudaGetLastError();
+    delete fe;
+    return HOUGH_OK;
+}
+
+int hough_frontend_slice(hough_frontend_t* fe, const float* d_x, const float* d_y, const float* d_z, const float* d_t,
+                         const int64_t* d_fill_offsets, int32_t n_fills, int64_t n_hits, float* d_u, float* d_v, int32_t* d_src,
+                         int64_t* d_offsets, int64_t capacity, void* stream)
+{
+    if (!fe || !d_fill_offsets || !d_offsets || n_fills < 0 || n_hits < 0 || capacity < 0) return HOUGH_EINVAL;
+    if (n_fills > fe->desc.max_fills || n_hits > fe->desc.max_hits) return HOUGH_ERANGE;
+    if (n_hits > 0 && (!d_x || !d_y || !d_z || !d_t)) return HOUGH_EINVAL;
+    if (capacity > 0 && (!d_u || !d_v || !d_src)) return HOUGH_EINVAL;
+    if (((uintptr_t)d_fill_offsets & 7) || ((uintptr_t)d_offsets & 7)) return HOUGH_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(fe->desc.device));
+    const long long nw = (long long)n_fills * fe->desc.windows_per_fill;
+    if (nw == 0) { HCK(cudaMemsetAsync(d_offsets, 0, 8, st)); return HOUGH_OK; }
+    HCK(cudaMemsetAsync(fe->FP.counts, 0, (size_t)nw * 4, st));
+    if (n_hits > 0) {
+        long long blocks = (n_hits + 255) / 256;
+        const long long cap = (long long)fe->n_sm * 16;
+        if (blocks > cap) blocks = cap;
+        HOUGH_LAUNCH(hough::fe_count_kernel, (int)blocks, 256, 0, st, fe->FP, d_x, d_y, d_z, d_t,
+                     reinterpret_cast<const long long*>(d_fill_offsets), n_fills, (long long)n_hits);
+        HCK(cudaGetLastError());
+    }
+    HOUGH_LAUNCH(hough::fe_scan_kernel, 1, 1024, 0, st, fe->FP, nw, reinterpret_cast<long long*>(d_offsets));
+    HCK(cudaGetLastError());
+    if (n_hits > 0) {
+        int blocks = (n_fills + 3) / 4;  // four warps per CTA, one warp per fill
+        if (blocks > fe->n_sm * 16) blocks = fe->n_sm * 16;
+        HOUGH_LAUNCH(hough::fe_scatter_kernel, blocks, 128, 0, st, fe->FP, d_z, reinterpret_cast<const long long*>(d_fill_offsets), n_fills,
+                     d_u, d_v, d_src, (long long)capacity);
+        HCK(cudaGetLastError());
+    }
+    return HOUGH_OK;
+}
+
+int hough_frontend_status(hough_frontend_t* fe, int32_t* out, void* stream)
+{
+    if (!fe || !out) return HOUGH_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(fe->desc.device));
+    HCK(cudaMemcpyAsync(out, fe->FP.status, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    HCK(cudaMemsetAsync(fe->FP.status, 0, sizeof(int32_t), st));
+    HCK(cudaStreamSynchronize(st));
     return HOUGH_OK;
 }
 

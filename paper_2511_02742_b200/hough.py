@@ -33,7 +33,9 @@ CANDIDATE_WORDS = 8   # a record is 8 x 32-bit words; device tensors of records 
 
 EXPORTS = ("hough_plan_create", "hough_plan_destroy", "hough_vote", "hough_find_clusters", "hough_assign_hits",
            "hough_run_host", "hough_run_host_chunked", "hough_plan_query", "hough_plan_status", "hough_plan_launch_count", "hough_plan_debug_counters",
-           "hough_measure_smem_atomic_peak", "hough_strerror", "hough_last_cuda_error", "hough_version")
+           "hough_measure_smem_atomic_peak", "hough_strerror", "hough_last_cuda_error", "hough_version",
+           "hough_refit_tracks", "hough_frontend_create", "hough_frontend_destroy", "hough_frontend_slice",
+           "hough_frontend_status")
 
 
 class hough_plan_desc_t(ctypes.Structure):
@@ -51,6 +53,24 @@ class hough_plan_info_t(ctypes.Structure):
                                               "n_ctas", "smem_bytes_per_cta", "n_sm", "fast_groups", "fast_threads",
                                               "fast_ctas", "fast_smem_bytes", "fast_hits_cap", "fast_on_cap", "fast_peak_cap",
                                               "fast_strip_list_cap")]
+
+
+# numpy view of hough_fit_t (32 bytes); device tensors of fit records are int32 [E, K, 8]
+FIT_DTYPE = np.dtype([("n_hits", "<i4"), ("max_run", "<i4"), ("plane_mask", "<u8"), ("slope", "<f4"), ("intercept", "<f4"),
+                      ("flags", "<i4"), ("reserved", "<i4")])
+HOUGH_FIT_FOUND, HOUGH_FIT_DEGENERATE = 1, 2
+HOUGH_STATUS_OUTPUT_TRUNCATED = 8
+
+
+class hough_plane_geometry_t(ctypes.Structure):
+    _fields_ = [("plane_origin", ctypes.c_double), ("plane_pitch", ctypes.c_double), ("n_planes", ctypes.c_int32),
+                ("min_run", ctypes.c_int32), ("wrap", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+class hough_frontend_desc_t(ctypes.Structure):
+    _fields_ = [("t0", ctypes.c_double), ("window_width", ctypes.c_double), ("window_step", ctypes.c_double),
+                ("windows_per_fill", ctypes.c_int32), ("xy_max", ctypes.c_double), ("max_fills", ctypes.c_int32),
+                ("max_hits", ctypes.c_int64), ("device", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 class HoughError(RuntimeError):
@@ -94,6 +114,11 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     L.hough_last_cuda_error.argtypes = []
     L.hough_last_cuda_error.restype = ctypes.c_char_p
     L.hough_version.argtypes = []
+    L.hough_refit_tracks.argtypes = [vp, vp, vp, vp, i32, vp, vp, ctypes.POINTER(hough_plane_geometry_t), vp, vp]
+    L.hough_frontend_create.argtypes = [ctypes.POINTER(hough_frontend_desc_t), ctypes.POINTER(vp)]
+    L.hough_frontend_destroy.argtypes = [vp]
+    L.hough_frontend_slice.argtypes = [vp, vp, vp, vp, vp, vp, i32, i64, vp, vp, vp, vp, i64, vp]
+    L.hough_frontend_status.argtypes = [vp, ctypes.POINTER(i32), vp]
     for name in EXPORTS:
         if name not in ("hough_strerror", "hough_last_cuda_error", "hough_plan_launch_count"):
             getattr(L, name).restype = ctypes.c_int
@@ -289,3 +314,83 @@ def plan_for_workload(wl, n_events: int, n_hits: int, max_hits_per_event: int, d
     return hough_plan_create(wl.n_theta, wl.n_rho, wl.rho_min, wl.rho_max, wl.coord_max, wl.vote_threshold, wl.assign_window,
                              wl.max_candidates, max(1, n_events), max(0, n_hits), max_hits_per_event,
                              HOUGH_U16 if wl.count_dtype == "u16" else HOUGH_I32, wl.hit_frac_bits, -1, device, flags)
+
+
+def hough_refit_tracks(plan: Plan, u: torch.Tensor, v: torch.Tensor, offsets: torch.Tensor, n_found: torch.Tensor,
+                       labels: torch.Tensor, plane_origin: float, plane_pitch: float, n_planes: int, min_run: int = 5,
+                       wrap: bool = False, fits: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """fits int32 [E, K, 8] -- the 32-byte hough_fit_t records as words (see fits_to_numpy); rows beyond min(n_found, K) untouched."""
+    E = _n_events(offsets)
+    if fits is None:
+        fits = torch.zeros((E, plan.K, 8), dtype=torch.int32, device=plan.device)
+    g = hough_plane_geometry_t(plane_origin, plane_pitch, n_planes, min_run, int(bool(wrap)), 0)
+    _check(load_library().hough_refit_tracks(plan.handle, _dev(plan, u, torch.float32, "u"), _dev(plan, v, torch.float32, "v"),
+                                             _dev(plan, offsets, torch.int64, "offsets"), E, _dev(plan, n_found, torch.int32, "n_found"),
+                                             _dev(plan, labels, torch.int32, "labels"), ctypes.byref(g),
+                                             _dev(plan, fits, torch.int32, "fits"), _stream_ptr(plan, stream)), "hough_refit_tracks")
+    return fits
+
+
+def fits_to_numpy(fits: torch.Tensor) -> np.ndarray:
+    """int32 [E, K, 8] tensor -> numpy structured array [E, K] of FIT_DTYPE (a copy on the host)."""
+    a = np.ascontiguousarray(fits.detach().cpu().numpy())
+    return a.view(FIT_DTYPE).reshape(a.shape[0], a.shape[1])
+
+
+class FrontEnd:
+    """Owner of a hough_frontend_t* (time slicing + phi = atan2(y, x))."""
+
+    def __init__(self, handle: int, desc: hough_frontend_desc_t):
+        self.handle = ctypes.c_void_p(handle)
+        self.desc = desc
+        self.device = torch.device("cuda", desc.device)
+        self.windows_per_fill = desc.windows_per_fill
+
+    def __del__(self):
+        try:
+            hough_frontend_destroy(self)
+        except Exception:
+            pass
+
+
+def hough_frontend_create(t0: float, window_width: float, window_step: float, windows_per_fill: int, max_fills: int,
+                          max_hits: int, xy_max: float = 512.0, device: int = 0) -> FrontEnd:
+    d = hough_frontend_desc_t(t0, window_width, window_step, windows_per_fill, xy_max, max_fills, max_hits, device, 0)
+    h = ctypes.c_void_p()
+    _check(load_library().hough_frontend_create(ctypes.byref(d), ctypes.byref(h)), "hough_frontend_create")
+    return FrontEnd(h.value, d)
+
+
+def hough_frontend_destroy(fe: FrontEnd) -> None:
+    if fe.handle is not None and fe.handle.value:
+        h, fe.handle = fe.handle, None
+        _check(load_library().hough_frontend_destroy(h), "hough_frontend_destroy")
+
+
+def hough_frontend_slice(fe: FrontEnd, x: torch.Tensor, y: torch.Tensor, z: torch.Tensor, t: torch.Tensor,
+                         fill_offsets: torch.Tensor, capacity: Optional[int] = None, stream=None):
+    """(u [capacity] fp32, v [capacity] fp32, src [capacity] int32, offsets [n_fills * windows_per_fill + 1] int64) on the device.
+    Only the first offsets[-1] entries of u, v, src are meaningful; capacity defaults to ceil(width / step) * n_hits."""
+    n_fills = _n_events(fill_offsets)
+    n = x.numel()
+    if capacity is None:
+        capacity = n * int(-(-fe.desc.window_width // fe.desc.window_step))
+    u = torch.empty(max(capacity, 1), dtype=torch.float32, device=fe.device)
+    v = torch.empty(max(capacity, 1), dtype=torch.float32, device=fe.device)
+    src = torch.empty(max(capacity, 1), dtype=torch.int32, device=fe.device)
+    offsets = torch.empty(n_fills * fe.windows_per_fill + 1, dtype=torch.int64, device=fe.device)
+    s = stream if stream is not None else torch.cuda.current_stream(fe.device)
+    _check(load_library().hough_frontend_slice(fe.handle, _dev(fe, x, torch.float32, "x"), _dev(fe, y, torch.float32, "y"),
+                                               _dev(fe, z, torch.float32, "z"), _dev(fe, t, torch.float32, "t"),
+                                               _dev(fe, fill_offsets, torch.int64, "fill_offsets"), n_fills, n,
+                                               ctypes.c_void_p(u.data_ptr()), ctypes.c_void_p(v.data_ptr()),
+                                               ctypes.c_void_p(src.data_ptr()), ctypes.c_void_p(offsets.data_ptr()), capacity,
+                                               ctypes.c_void_p(s.cuda_stream)), "hough_frontend_slice")
+    return u, v, src, offsets
+
+
+def hough_frontend_status(fe: FrontEnd, stream=None) -> int:
+    out = ctypes.c_int32(0)
+    s = stream if stream is not None else torch.cuda.current_stream(fe.device)
+    _check(load_library().hough_frontend_status(fe.handle, ctypes.byref(out), ctypes.c_void_p(s.cuda_stream)), "hough_frontend_status")
+    return out.value

@@ -128,6 +128,7 @@ static inline double __ddiv_rn(double a, double b) { return a / b; }
 static inline double __dadd_rn(double a, double b) { return a + b; }
 static inline int __popc(unsigned x) { return __builtin_popcount(x); }
 static inline int __ffs(unsigned x) { return __builtin_ffs((int)x); }
+static inline int __ffsll(long long x) { return __builtin_ffsll(x); }
 static inline int __clz(unsigned x) { return x ? __builtin_clz(x) : 32; }
 static inline long long clock64() { return 0; }
 static inline unsigned __vmaxu2(unsigned a, unsigned b)

@@ -158,3 +158,76 @@ def run_host(p, u, v, offsets, n_chunks, count_dtype=HOUGH_I32, repeat=1):
                emu_violations=int(L.cuda_emu_violations()), emu_first_violation=L.cuda_emu_first_violation().decode())
     L.hough_plan_destroy(h)
     return out
+
+
+# ----------------------------------------------------------------------------- stages around the core
+FIT_DTYPE = np.dtype([("n_hits", "<i4"), ("max_run", "<i4"), ("plane_mask", "<u8"), ("slope", "<f4"), ("intercept", "<f4"),
+                      ("flags", "<i4"), ("reserved", "<i4")])
+assert FIT_DTYPE.itemsize == 32
+
+
+class PlaneGeometry(ctypes.Structure):
+    _fields_ = [("plane_origin", ctypes.c_double), ("plane_pitch", ctypes.c_double), ("n_planes", ctypes.c_int32),
+                ("min_run", ctypes.c_int32), ("wrap", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+class FrontDesc(ctypes.Structure):
+    _fields_ = [("t0", ctypes.c_double), ("window_width", ctypes.c_double), ("window_step", ctypes.c_double),
+                ("windows_per_fill", ctypes.c_int32), ("xy_max", ctypes.c_double), ("max_fills", ctypes.c_int32),
+                ("max_hits", ctypes.c_int64), ("device", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+def refit(p, u, v, offsets, n_found, labels, geom, count_dtype=HOUGH_I32, max_hpe=None):
+    """hough_refit_tracks on the emulated device -> (fits [E][K] structured array, return code)."""
+    L = lib()
+    L.cuda_emu_reset_violations()
+    vp, i32 = ctypes.c_void_p, ctypes.c_int32
+    L.hough_refit_tracks.argtypes = [vp, vp, vp, vp, i32, vp, vp, ctypes.POINTER(PlaneGeometry), vp, vp]
+    E = len(offsets) - 1
+    hpe = int(np.diff(offsets).max()) if E > 0 and len(u) else 0
+    d = Desc(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.hit_frac_bits, p.acc_frac_bits, p.vote_threshold,
+             p.assign_window, p.max_candidates, count_dtype, max(1, E), max(0, len(u)), max(hpe, 1) if max_hpe is None else max_hpe, 0, 0)
+    h = ctypes.c_void_p()
+    assert L.hough_plan_create(ctypes.byref(d), ctypes.byref(h)) == 0
+    du, dv, do = DevBuf(np.asarray(u, np.float32)), DevBuf(np.asarray(v, np.float32)), DevBuf(np.asarray(offsets, np.int64))
+    dn, dl = DevBuf(np.asarray(n_found, np.int32)), DevBuf(np.asarray(labels, np.int32))
+    fits = DevBuf(np.zeros((E, p.max_candidates), FIT_DTYPE))
+    g = PlaneGeometry(geom.origin, geom.pitch, geom.n_planes, geom.min_run, int(geom.wrap), 0)
+    rc = L.hough_refit_tracks(h, du.ptr, dv.ptr, do.ptr, E, dn.ptr, dl.ptr, ctypes.byref(g), fits.ptr, None)
+    dbg = np.zeros(16, np.uint64)
+    L.hough_plan_debug_counters(h, dbg.ctypes.data, None)
+    L.hough_plan_destroy(h)
+    assert L.cuda_emu_violations() == 0, L.cuda_emu_first_violation().decode()
+    assert int(dbg[14]) == 0, f"index check failed at site {int(dbg[13])}"
+    return fits.view.copy(), rc
+
+
+def frontend_slice(fe, x, y, z, t, fill_offsets, capacity=None):
+    """hough_frontend_* on the emulated device.  fe: oracle.track_def.FrontEnd (field names only; no arithmetic is shared).
+    -> dict(u, v, src, offsets, status)"""
+    L = lib()
+    L.cuda_emu_reset_violations()
+    vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+    L.hough_frontend_create.argtypes = [ctypes.POINTER(FrontDesc), ctypes.POINTER(vp)]
+    L.hough_frontend_destroy.argtypes = [vp]
+    L.hough_frontend_slice.argtypes = [vp, vp, vp, vp, vp, vp, i32, i64, vp, vp, vp, vp, i64, vp]
+    L.hough_frontend_status.argtypes = [vp, ctypes.POINTER(i32), vp]
+    n_fills, n = len(fill_offsets) - 1, len(x)
+    d = FrontDesc(fe.t0, fe.width, fe.step, fe.windows_per_fill, fe.xy_max, max(1, n_fills), n, 0, 0)
+    h = vp()
+    rc = L.hough_frontend_create(ctypes.byref(d), ctypes.byref(h))
+    assert rc == 0, f"hough_frontend_create -> {rc}"
+    m = -(-int(round(fe.width * 256)) // int(round(fe.step * 256)))
+    cap = m * n if capacity is None else capacity
+    bx, by, bz, bt = (DevBuf(np.asarray(a, np.float32)) for a in (x, y, z, t))
+    bf = DevBuf(np.asarray(fill_offsets, np.int64))
+    bu, bv = DevBuf(np.full(cap, np.nan, np.float32)), DevBuf(np.full(cap, np.nan, np.float32))
+    bs = DevBuf(np.full(cap, -1, np.int32))
+    bo = DevBuf(np.full(n_fills * fe.windows_per_fill + 1, -1, np.int64))
+    rc = L.hough_frontend_slice(h, bx.ptr, by.ptr, bz.ptr, bt.ptr, bf.ptr, n_fills, n, bu.ptr, bv.ptr, bs.ptr, bo.ptr, cap, None)
+    assert rc == 0, f"hough_frontend_slice -> {rc}"
+    st = i32(0)
+    L.hough_frontend_status(h, ctypes.byref(st), None)
+    L.hough_frontend_destroy(h)
+    assert L.cuda_emu_violations() == 0, L.cuda_emu_first_violation().decode()
+    return dict(u=bu.view.copy(), v=bv.view.copy(), src=bs.view.copy(), offsets=bo.view.copy(), status=st.value)

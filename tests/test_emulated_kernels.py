@@ -21,7 +21,7 @@ from oracle import hough_c as C  # noqa: E402
 from oracle import hough_def as D  # noqa: E402
 from paper_2511_02742_b200 import synth  # noqa: E402
 from test_oracle_pins import edge_cases  # noqa: E402
-from util import mixed_batch, paper_grid_batch, params_of, std_params  # noqa: E402
+from util import fills_with_tracks, mixed_batch, paper_grid_batch, params_of, std_params, synthetic_fills  # noqa: E402
 
 INT_FIELDS = ("theta_bin", "rho_bin", "votes", "cluster_root", "cluster_nbins", "reserved")
 
@@ -273,3 +273,95 @@ def test_run_host_chunked(n_chunks, n_events):
     for e in range(len(offsets) - 1):
         k = min(int(o["n_found"][e]), p.max_candidates)
         assert g["cands"][e, :k].tobytes() == o["cands"][e, :k].tobytes()
+
+
+# ----------------------------------------------------------------------------- stages around the core (O9-O12)
+from oracle import track_def as T  # noqa: E402
+
+GEOM = T.PlaneGeometry(origin=-94.0, pitch=4.0, n_planes=48)
+
+
+def fits_equal(fits_row, oracle_fits):
+    for s, f in enumerate(oracle_fits):
+        g = fits_row[s]
+        assert (int(g["n_hits"]), int(g["plane_mask"]), int(g["max_run"]), int(g["flags"]), int(g["reserved"])) == \
+               (f.n_hits, f.plane_mask, f.max_run, f.flags, 0), (s, g, f)
+        assert g["slope"].tobytes() == f.slope.tobytes() and g["intercept"].tobytes() == f.intercept.tobytes(), (s, g, f)
+
+
+@pytest.mark.parametrize("cfg,n_events,geom", [(1, 12, GEOM), (3, 3, GEOM), (2, 5, T.PlaneGeometry(-94.0, 4.0, 48, min_run=7, wrap=True))])
+def test_refit_tracks(cfg, n_events, geom):
+    """O9 + O10: per kept candidate the exact integer sums, plane mask, longest run and the line, bit for bit."""
+    wl = synth.workload(cfg)
+    b = synth.generate(wl, 0, n_events)
+    p = params_of(wl)
+    o = C.run_batch(b.u, b.v, b.offsets, p)
+    fits, rc = E.refit(p, b.u, b.v, b.offsets, o["n_found"], o["labels"], geom, dtype_of(wl))
+    assert rc == 0
+    for e in range(n_events):
+        a, z = int(b.offsets[e]), int(b.offsets[e + 1])
+        nk = min(int(o["n_found"][e]), p.max_candidates)
+        fits_equal(fits[e], T.refit_event(b.u[a:z], b.v[a:z], o["labels"][a:z], nk, p, geom))
+        assert (fits[e, nk:]["n_hits"] == 0).all()                       # rows beyond n_kept are untouched
+
+
+def test_refit_rejects_plans_whose_sums_could_overflow():
+    p = D.Params(64, 512, -1415.0, 1415.0, 1000.0, 3, 6.0, 16, 6, -1)    # coord_max 2^H = 64000 > 2^15
+    u = np.zeros(4, np.float32)
+    _, rc = E.refit(p, u, u, np.array([0, 4], np.int64), np.zeros(1, np.int32), np.full(4, -1, np.int32), GEOM)
+    assert rc == -2
+
+
+@pytest.mark.parametrize("fe", [T.FrontEnd(windows_per_fill=12), T.FrontEnd(t0=-3.5, width=10.0, step=2.5, windows_per_fill=20),
+                                T.FrontEnd(t0=1.0, width=4.0, step=6.0, windows_per_fill=7)],
+                         ids=["10ns_5ns", "four_fold_overlap", "gaps_between_windows"])
+def test_frontend_slice(fe):
+    """O11 + O12: window membership, input order inside a window, CORDIC phi and the event offsets, bit for bit."""
+    x, y, z, t, fo = synthetic_fills(5, seed=41)
+    ou, ov, osrc, ooff = T.slice_batch(x, y, z, t, fo, fe)
+    g = E.frontend_slice(fe, x, y, z, t, fo)
+    assert g["status"] == 0
+    np.testing.assert_array_equal(g["offsets"], ooff)
+    M = int(ooff[-1])
+    assert M > 0
+    np.testing.assert_array_equal(g["src"][:M], osrc)
+    assert g["u"][:M].tobytes() == ou.tobytes() and g["v"][:M].tobytes() == ov.tobytes()
+    assert (g["src"][M:] == -1).all()                                       # nothing is written past the last window
+
+
+def test_frontend_reports_truncation_and_still_writes_all_offsets():
+    fe = T.FrontEnd(windows_per_fill=12)
+    x, y, z, t, fo = synthetic_fills(3, seed=42)
+    _, _, osrc, ooff = T.slice_batch(x, y, z, t, fo, fe)
+    cap = int(ooff[-1]) // 2
+    g = E.frontend_slice(fe, x, y, z, t, fo, capacity=cap)
+    assert g["status"] & 8
+    np.testing.assert_array_equal(g["offsets"], ooff)
+    np.testing.assert_array_equal(g["src"][:cap], osrc[:cap])
+
+
+def test_frontend_feeds_the_hough_core():
+    """Fills -> windows -> vote / clusters / assign -> refit, every stage against its oracle on the previous stage's output."""
+    fe = T.FrontEnd(windows_per_fill=6)
+    x, y, z, t, fo = fills_with_tracks(3, seed=43)
+    g = E.frontend_slice(fe, x, y, z, t, fo)
+    ou, ov, osrc, ooff = T.slice_batch(x, y, z, t, fo, fe)
+    M = int(ooff[-1])
+    np.testing.assert_array_equal(g["offsets"], ooff)
+    assert g["u"][:M].tobytes() == ou.tobytes()
+    p = D.Params(180, 1000, -500.0, 500.0, 256.0, 12, 2.0, 8)               # the paper's grid (PAPER.md L106)
+    h = E.run(p, g["u"][:M], g["v"][:M], g["offsets"], want_acc=False)
+    o = oracle_run(p, ou, ov, ooff, want_acc=False)
+    assert_same(h, o, p)
+    assert (o["n_found"] >= 1).sum() >= 3                                   # the windows that hold a track find it
+    vanes40 = T.PlaneGeometry(origin=-175.5, pitch=9.0, n_planes=40, min_run=5, wrap=True)
+    fits, rc = E.refit(p, ou, ov, ooff, o["n_found"], o["labels"], vanes40)
+    assert rc == 0
+    found = 0
+    for e in range(len(ooff) - 1):
+        a, zz = int(ooff[e]), int(ooff[e + 1])
+        nk = min(int(o["n_found"][e]), p.max_candidates)
+        fo_e = T.refit_event(ou[a:zz], ov[a:zz], o["labels"][a:zz], nk, p, vanes40)
+        fits_equal(fits[e], fo_e)
+        found += sum(1 for f in fo_e if f.flags & T.FIT_FOUND)
+    assert found >= 3

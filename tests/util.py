@@ -93,3 +93,45 @@ def paper_grid_batch(n_events, seed=31):
         pm = rng.permutation(len(uu))
         us.append(uu[pm]); vs.append(vv[pm]); offs.append(offs[-1] + len(uu))
     return p, np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64)
+
+
+def synthetic_fills(n_fills, seed, hits_per_fill=600, t_span=80.0):
+    """RecoHits of a few fills: points on the 40 radial vanes (r from 70 to 290 mm, z within +-200 mm), times
+    uniform over the fill, some invalid ones; in no particular order."""
+    rng = np.random.default_rng(seed)
+    xs, ys, zs, ts, fo = [], [], [], [], [0]
+    for f in range(n_fills):
+        n = int(rng.integers(hits_per_fill // 2, hits_per_fill + 1)) if f != 1 else 0
+        vane = rng.integers(0, 40, n)
+        r = rng.uniform(70.0, 290.0, n)
+        ang = np.radians(vane * 9.0 + 4.5)
+        x, y = r * np.cos(ang), r * np.sin(ang)
+        z, t = rng.uniform(-200, 200, n), rng.uniform(-15.0, t_span, n)
+        if n > 8:
+            x[3], t[5], z[6] = np.nan, np.inf, -np.inf
+            x[7] = y[7] = 0.0
+            x[8] = 600.0
+            t[9] = 5.0                                                      # exactly on a window edge
+        xs.append(x); ys.append(y); zs.append(z); ts.append(t); fo.append(fo[-1] + n)
+    cat = lambda a: np.concatenate(a).astype(np.float32)
+    return cat(xs), cat(ys), cat(zs), cat(ts), np.array(fo, np.int64)
+
+
+def fills_with_tracks(n_fills, seed, tracks_per_fill=2):
+    """RecoHits of fills that hold helix-like tracks: phi (degrees) linear in z, one hit per crossed vane, all hits of a track
+    within one ns of each other (a helix projected onto the phi-z plane is a straight line)."""
+    rng = np.random.default_rng(seed)
+    xs, ys, zs, ts, fo = [], [], [], [], [0]
+    for f in range(n_fills):
+        n_f = 0
+        for trk in range(tracks_per_fill):
+            z0, slope, t_trk = rng.uniform(-100, 100), rng.uniform(-0.8, 0.8), rng.uniform(8, 22)
+            vanes = np.arange(int(rng.integers(0, 10)), int(rng.integers(20, 40)))
+            phi = np.radians(vanes * 9.0 + 4.5 - 180.0)
+            r = rng.uniform(100, 280, len(vanes))
+            xs.append(r * np.cos(phi)); ys.append(r * np.sin(phi)); zs.append(z0 + slope * (vanes * 9.0 - 180.0))
+            ts.append(np.full(len(vanes), t_trk) + rng.uniform(-0.5, 0.5, len(vanes)))
+            n_f += len(vanes)
+        fo.append(fo[-1] + n_f)
+    x, y, z, t = (np.concatenate(a).astype(np.float32) for a in (xs, ys, zs, ts))
+    return x, y, z, t, np.array(fo, np.int64)
