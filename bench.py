@@ -2,6 +2,9 @@
 """bench.py -- throughput of the batched Hough track-finding hot path on B200 (contract: see DESIGN.md "Measurement").
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--cfg 3] [--events E]
+    python bench.py --gpus N                      # N > 1 without a launcher: bench.py starts the N ranks itself (torchrun)
+    python bench.py --gpus N --scaling strong     # one batch cut over the ranks by hit count (default: weak, own events per rank)
+    python bench.py --all-configs [--out FILE]    # one JSON line per BASELINE config 0, 1, 2 and per cell of the config-4 sweep
 
 A "step" is one pass of the whole hot path (hough_find_clusters + hough_assign_hits) over one batch of synthetic events
 of BASELINE.json's high-pile-up config (configs[3]: 100,000 events, ~2,784 hits each, 512 x 512 accumulator).  One JSON
@@ -186,17 +189,30 @@ def run_reference(args):
     return 0
 
 
-def run_ours(args):
+def run_ours(args, cfg=None, hits_idx=None, grid_idx=None, quiet=False):
+    """One workload on this rank's GPU; rank 0 returns (and, unless quiet, prints) the JSON line."""
     rank, world, local_rank = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
-    wl = synth.workload(args.cfg, args.hits_idx, args.grid_idx)
-    if world > 1:
+    wl = synth.workload(args.cfg if cfg is None else cfg, args.hits_idx if hits_idx is None else hits_idx,
+                        args.grid_idx if grid_idx is None else grid_idx)
+    strong = world > 1 and args.scaling == "strong"
+    if world > 1 and not strong:
         import dataclasses
         wl = dataclasses.replace(wl, cell=wl.cell + 16 * rank)       # weak scaling: every rank gets its own events (own RNG stream)
     n_events = min(args.events or wl.n_events, wl.n_events)
+    if args.max_hits and wl.hits_per_event_nominal * n_events > args.max_hits:
+        n_events = max(1000, int(args.max_hits // wl.hits_per_event_nominal) // 1000 * 1000)
     procs = max(1, (os.cpu_count() or 1) // max(1, env_int("LOCAL_WORLD_SIZE", world)))
     t_gen = time.perf_counter()
     u, v, offsets = generate_parallel(wl, n_events, procs=min(procs, 32))    # before CUDA is initialised (fork)
     t_gen = time.perf_counter() - t_gen
+    shard_ranges = None
+    if strong:
+        # strong scaling: ONE batch, cut into contiguous event ranges balanced by hit count; no collective on the data path
+        from paper_2511_02742_b200 import shard
+        shard_ranges = shard.shard_events(offsets, world)
+        u, v, offsets = shard.local_batch(u, v, offsets, shard_ranges[rank])
+        u, v = np.ascontiguousarray(u), np.ascontiguousarray(v)
+        n_events = len(offsets) - 1
     n_hits = int(offsets[-1])
     max_hpe = int(np.diff(offsets).max()) if n_events else 1
 
@@ -301,6 +317,13 @@ def run_ours(args):
                "same_as_device_results": bool((hn == n_found.cpu()).all().item() and (hl == labels.cpu()).all().item())}
         del hc, hl
 
+    gathered = None
+    if strong:
+        # per-event results back in event order on every rank (NCCL all-gather; outside the timed region: the data path has no collective)
+        from paper_2511_02742_b200 import shard
+        gathered = shard.gather_per_event(n_found, shard_ranges)
+        assert gathered.numel() == sum(b - a for a, b in shard_ranges)
+
     line = None
     if rank == 0:
         # ---- roofline of the dominant kernel (fused vote + peak/cluster finding): shared-memory atomic adds
@@ -321,7 +344,13 @@ def run_ours(args):
                     "alu_issue": {"peak": alu_peak / 1e9, "unit": "Gvote/s", "frac": achieved / alu_peak,
                                   "note": "5 issue slots per vote x 4 schedulers x n_sm x sm_max_mhz (DESIGN.md)"},
                     "ms_per_launch": ms_find, "share_of_step": ms_find / (ms_find + ms_assign),
-                    "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(wl.name) if n_events == wl.n_events else None,
+                    # the reported fraction of the whole pipeline (find + assign) next to the dominant kernel's
+                    "frac_pipeline": votes_launch / ((ms_find + ms_assign) * 1e-3) / peak_ops,
+                    # second, diagnostic ceiling for sparse workloads: every tile byte is zeroed and scanned once per event
+                    # at 128 B / clk / SM of shared-memory bandwidth (u16 or i32 counters as the plan chose)
+                    "dense_tile": dense_tile_ceiling(info, wl, sm_max, n_events / (ms_find * 1e-3)),
+                    "traffic": traffic_from_profiles(wl.name, "hough_fast_kernel" if info["fast_groups"] else "hough_event_kernel")
+                    if n_events == wl.n_events else None,
                     "hbm": {"algorithmic_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / (ms_find * 1e-3) / 1e9,
                             "peak_gbs": hbm_peak, "peak_source": "MEASURED_PEAKS.json" if hbm_peak else "absent",
                             "frac": (hbm_bytes / (ms_find * 1e-3) / 1e9 / hbm_peak) if hbm_peak else None}}
@@ -340,24 +369,90 @@ def run_ours(args):
                    "sample": f"first {ns} events of the workload, {dt:.1f} s, oracle/hough_oracle.c single thread",
                    "gpu_outputs_identical_on_sample": same}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32",
+                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None,
+                "dtype": "int32",
                 "data": "synthetic", "votes_per_s": votes_per_s,
-                "config": config_of(wl, n_events, n_hits, {"parallelism": f"events sharded over {world} GPU(s), no collective",
-                                                           "plan": info, "status_word": status, "gen_s": round(t_gen, 1)}),
+                "config": config_of(wl, int(events_all) if strong else n_events, int(hits_all) if strong else n_hits,
+                                    {"parallelism": (f"one batch cut into {world} contiguous event ranges balanced by hit count "
+                                                     "(shard.shard_events), no collective on the data path; per-event results "
+                                                     "all-gathered afterwards" if strong else
+                                                     f"events sharded over {world} GPU(s), no collective"),
+                                     "plan": info, "status_word": status, "gen_s": round(t_gen, 1)}),
                 "kernel_ms": {"hough_find_clusters": ms_find, "hough_assign_hits": ms_assign},
                 "ms_per_step_median": statistics.median(step_ms), "ms_per_step_best": min(step_ms),     # this rank's steps
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
     H.hough_plan_destroy(plan)
     if dist is not None:
         dist.destroy_process_group()
-    if line is not None:
+    if line is not None and not quiet:
         print(json.dumps(line), flush=True)
+    return line
+
+
+def traffic_from_profiles(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on `workload`, read from the committed ncu table
+    profiles/ncu_traffic.csv (one row per `ncu --set full` capture; the newest row wins); None if no capture exists."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    best = None
+    try:
+        with open(path) as f:
+            header = f.readline().strip().split(",")
+            for row in f:
+                r = dict(zip(header, row.strip().split(",")))
+                if r.get("workload") == workload and r.get("kernel", "").startswith(kernel):
+                    best = int(r["dram_bytes_read"]) + int(r["dram_bytes_write"])
+    except (OSError, ValueError, KeyError):
+        return None
+    return best
+
+
+def dense_tile_ceiling(info, wl, sm_hz, events_per_s):
+    tile_bytes = wl.n_theta * wl.n_rho * (2 if info["fast_groups"] else info["counter_bytes"])
+    peak = info["n_sm"] * sm_hz * 128.0 / (2.0 * tile_bytes)
+    return {"peak_events_per_s": peak, "frac": events_per_s / peak, "tile_bytes_per_event": tile_bytes}
+
+
+ALL_CONFIGS = [(0, 0, 0), (1, 0, 0), (2, 0, 0)] + [(4, h, g) for h in range(4) for g in range(4)]
+
+
+def run_all_configs(args):
+    """One JSON line per BASELINE config 0, 1, 2 and per cell of the config-4 roofline sweep, written to
+    --out; the default bench line (config 3) is not part of this mode.  Single GPU."""
+    if env_int("WORLD_SIZE", 1) != 1:
+        print("bench.py --all-configs runs on one GPU", file=sys.stderr)
+        return 2
+    out = args.out or os.path.join(ROOT, "gpurun_out", "all_configs.jsonl")
+    os.makedirs(os.path.dirname(out), exist_ok=True)
+    args.no_e2e = True
+    args.cpu_events = min(args.cpu_events, 64)
+    n = 0
+    with open(out, "w") as f:
+        for cfg, h, g in ALL_CONFIGS:
+            line = run_ours(args, cfg, h, g, quiet=True)
+            f.write(json.dumps(line) + "\n")
+            f.flush()
+            n += 1
+    print(json.dumps({"all_configs": n, "out": out}), flush=True)
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one hough_event_kernel launch, from the ncu --set full capture under
-# profiles/ (workload name -> bytes); None until a capture of that workload exists.
-TRAFFIC_BYTES_PER_LAUNCH = {"cfg3_100k_events_pileup40": 2637558016}   # dram read + write of one launch, profiles/r1_fast_kernel_ncu.md
+def free_port():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def launch_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks with torchrun on this node and wait for them."""
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        print(f"bench.py --gpus {args.gpus}: only {have} CUDA device(s) visible", file=sys.stderr)
+        return 2
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -374,9 +469,25 @@ def main():
     ap.add_argument("--ref-events", type=int, default=200, help="--impl reference: events per step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="N > 1: own events per rank, or one batch cut over the ranks")
+    ap.add_argument("--all-configs", action="store_true", help="configs 0, 1, 2 and the 16 cells of config 4, one JSON line each, to --out")
+    ap.add_argument("--out", default="", help="--all-configs: output file (default gpurun_out/all_configs.jsonl)")
+    ap.add_argument("--max-hits", type=float, default=0, help="cap a workload at about this many hits (fewer events; recorded in config)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    return run_reference(args) if args.impl == "reference" else run_ours(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is None and args.gpus > 1:
+        return launch_ranks(args)                                      # no launcher: start the ranks ourselves
+    if int(world_env or 1) != args.gpus:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world_env or 1}: launch one rank per GPU (or drop the launcher and let "
+              "bench.py start them)", file=sys.stderr)
+        return 2
+    if args.all_configs:
+        return run_all_configs(args)
+    run_ours(args)
+    return 0
 
 
 if __name__ == "__main__":

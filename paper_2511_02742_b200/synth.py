@@ -65,6 +65,19 @@ class Workload:
     hit_frac_bits: int = HIT_FRAC_BITS
     max_candidates: int = MAX_CANDIDATES
     assign_window_bins: float = 1.0   # w = assign_window_bins * d_rho
+    # detector geometry of the generator (defaults: the 48 planes of SURVEY.md Sec. 8(d))
+    n_planes: int = N_PLANES
+    plane_u0: float = PLANE_U0
+    plane_pitch: float = PLANE_PITCH
+    noise_u: float = NOISE_U
+    noise_v: float = NOISE_V
+
+    @property
+    def hits_per_event_nominal(self) -> float:
+        if self.hits_total is not None:
+            return float(self.hits_total)
+        n_tr = 0.5 * (self.tracks[0] + self.tracks[1])
+        return n_tr * self.n_planes * (1.0 - self.inefficiency) + np.floor(self.noise_frac * self.n_planes * n_tr + 0.5)
 
     @property
     def d_rho(self) -> float:
@@ -102,6 +115,13 @@ def workload(cfg: int, hits_idx: int = 0, grid_idx: int = 0) -> Workload:
         n_tr = max(1, int(np.floor(h / 96.0 + 0.5)))
         # threshold "0.4 x planes" = round(19.2) = 19 (reading A17)
         return Workload(f"cfg4_sweep_h{h}_g{g}", 4, hits_idx, 50000, (n_tr, n_tr), 0.1, 0.0, 0.0, h, g, g, 19, "i32")
+    if cfg == 5:
+        # The paper's own CPU grid (180 theta bins over 0-180 deg, 1000 rho bins over -500...500) with the
+        # detector's 40 vanes as planes in phi (L72; 9 degrees apart), z within +-200 mm, 10-30 tracks per 10 ns window
+        # (L156: up to 6 tracks / ns).  Not a BASELINE config: SURVEY.md 8(f) NEXT-4 "the paper's own 180 x 1000 workload".
+        return Workload("paper_grid_180x1000_40vanes", 5, 0, 20000, (10, 30), 0.1, 0.30, 0.05, None, 180, 1000, 16, "u16",
+                        rho_min=-500.0, rho_max=500.0, coord_max=360.0, n_planes=40, plane_u0=-175.5, plane_pitch=9.0,
+                        noise_u=180.0, noise_v=200.0)
     raise ValueError(f"unknown config {cfg}")
 
 
@@ -167,26 +187,26 @@ def generate_chunk(wl: Workload, chunk: int) -> EventBatch:
     n_tracks = int(n_tr.sum())
     m = rng.uniform(-1.0, 1.0, size=n_tracks)
     c = rng.uniform(-100.0, 100.0, size=n_tracks)
-    smear = rng.normal(0.0, wl.sigma, size=(n_tracks, N_PLANES))
-    keep = rng.random(size=(n_tracks, N_PLANES)) >= wl.inefficiency
-    planes = PLANE_U0 + PLANE_PITCH * np.arange(N_PLANES, dtype=np.float64)
+    smear = rng.normal(0.0, wl.sigma, size=(n_tracks, wl.n_planes))
+    keep = rng.random(size=(n_tracks, wl.n_planes)) >= wl.inefficiency
+    planes = wl.plane_u0 + wl.plane_pitch * np.arange(wl.n_planes, dtype=np.float64)
     v_tr = m[:, None] * planes[None, :] + c[:, None] + smear
     u_tr = np.broadcast_to(planes[None, :], v_tr.shape)
     if wl.hits_total is not None:
-        n_noise = wl.hits_total - N_PLANES * n_tr
+        n_noise = wl.hits_total - wl.n_planes * n_tr
         if (n_noise < 0).any():
             raise ValueError("hits_total smaller than the track hits")
     else:
-        n_noise = np.floor(wl.noise_frac * N_PLANES * n_tr + 0.5).astype(np.int64)
+        n_noise = np.floor(wl.noise_frac * wl.n_planes * n_tr + 0.5).astype(np.int64)
     nn = int(n_noise.sum())
-    nu = rng.uniform(-NOISE_U, NOISE_U, size=nn)
-    nv = rng.uniform(-NOISE_V, NOISE_V, size=nn)
+    nu = rng.uniform(-wl.noise_u, wl.noise_u, size=nn)
+    nv = rng.uniform(-wl.noise_v, wl.noise_v, size=nn)
 
     ev_of_track = np.repeat(np.arange(n_ev, dtype=np.int64), n_tr)
     track_in_event = np.arange(n_tracks, dtype=np.int64) - np.repeat(np.cumsum(n_tr) - n_tr, n_tr)
     kf = keep.ravel()
-    ev_th = np.repeat(ev_of_track, N_PLANES)[kf]
-    tid_th = np.repeat(track_in_event, N_PLANES)[kf]
+    ev_th = np.repeat(ev_of_track, wl.n_planes)[kf]
+    tid_th = np.repeat(track_in_event, wl.n_planes)[kf]
     ev_all = np.concatenate([ev_th, np.repeat(np.arange(n_ev, dtype=np.int64), n_noise)])
     u_all = np.concatenate([u_tr.ravel()[kf], nu])
     v_all = np.concatenate([v_tr.ravel()[kf], nv])
