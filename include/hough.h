@@ -172,6 +172,19 @@ int hough_refit_tracks(hough_plan_t* plan, const float* d_u, const float* d_v, c
                        const int32_t* d_n_found, const int32_t* d_labels, const hough_plane_geometry_t* geometry,
                        hough_fit_t* d_fits, void* stream);
 
+/* Variant: the paper's own peak rule, one track at a time.  PAPER.md L94, L106: "a peak-finding
+ * algorithm identifies the bin with the highest number of entries ... track seeds are found by selecting the hits that align
+ * with the straight line".  Per event, repeated up to K times: histogram of the remaining hits -> global maximum under the
+ * order (count descending, t * n_rho + r ascending); stop if its count < T; its hits (distance to the bin-centre line within
+ * the assignment window) get the track's number as label and leave the hit set; a maximum none of whose hits lies in the
+ * window ends the search.  K times the work of hough_find_clusters: for comparison, not for throughput.
+ *   d_cands    [n_events][K]: track s of event e in record s (cluster_root = s, cluster_nbins = 0)
+ *   d_n_found  [n_events]: number of tracks of the event
+ *   d_labels   [N]: track number of every hit, or -1 */
+int hough_find_tracks_peeloff(hough_plan_t* plan, const float* d_u, const float* d_v, const int64_t* d_offsets,
+                              int32_t n_events, hough_candidate_t* d_cands, int32_t* d_n_found, int32_t* d_labels,
+                              void* stream);
+
 /* Front end: RecoHits (x, y, z, t) of a batch of fills -> one event per time window, in the (phi, z) plane.
  * "the reconstructed hit points are divided into overlapping time windows of 10 ns, with a sliding step of
  * 5 ns.  Within each time window, the spatial coordinates (x, y, z) of the hits are transformed into the (phi, z) space".

@@ -790,6 +790,32 @@ int hough_refit_tracks(hough_plan_t* p, const float* d_u, const float* d_v, cons
     return HOUGH_OK;
 }
 
+// ---------------------------------------------------------------- variant: iterative global-maximum peel-off (hough_track.cuh)
+
+int hough_find_tracks_peeloff(hough_plan_t* p, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events,
+                              hough_candidate_t* d_cands, int32_t* d_n_found, int32_t* d_labels, void* stream)
+{
+    int rc = check_common(p, d_u, d_v, d_offsets, n_events);
+    if (rc) return rc;
+    if (!d_cands || !d_n_found || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_n_found & 3)) return HOUGH_EINVAL;
+    if (n_events == 0) return HOUGH_OK;
+    if (!d_labels && p->desc.max_hits > 0) return HOUGH_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(p->desc.device));
+    // theta rows per strip: as many i32 rows as fit 200 KB of shared memory
+    int S = (int)((200u * 1024u) / ((size_t)p->desc.n_rho * 4));
+    if (S > p->desc.n_theta) S = p->desc.n_theta;
+    if (S < 1) return HOUGH_ERANGE;
+    const size_t smem = (size_t)S * p->desc.n_rho * 4;
+    if (smem > 48 * 1024) HCK(cudaFuncSetAttribute(hough::hough_peel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int grid = n_events < p->info.n_sm ? n_events : p->info.n_sm;
+    HOUGH_LAUNCH(hough::hough_peel_kernel, grid, 512, smem, st, p->P, S, d_u, d_v, reinterpret_cast<const long long*>(d_offsets), n_events,
+                 reinterpret_cast<Candidate*>(d_cands), d_n_found, d_labels);
+    HCK(cudaGetLastError());
+    p->launches += 1;
+    return HOUGH_OK;
+}
+
 // ---------------------------------------------------------------- front end: time slicing + phi (hough_track.cuh)
 
 struct hough_frontend {

@@ -244,4 +244,109 @@ hough_refit_kernel(const DevParams P, const PlaneParams G, const float* __restri
     }
 }
 
+// ---------------------------------------------------------------- variant: iterative global-maximum peel-off (O13, reading B7)
+//
+// The paper's CPU peak rule ("a peak-finding algorithm identifies the bin with the highest number of
+// entries ... track seeds are found by selecting the hits that align with the straight line"), repeated on the hits that
+// remain.  One CTA per event; per track: the histogram of the remaining hits is refilled strip by strip (i32 counters in
+// shared memory, S theta rows at a time), the maximum under the total order (count, -L) is kept across strips, its hits
+// (|e| <= W_q) get the track's slot as label and leave the hit set.  labels[] doubles as the "removed" flag.  This variant
+// is K times the work of the one-pass search and exists for comparison, not for throughput.
+struct PeelShared {
+    unsigned long long best;   // (count << 32) | (0xffffffff - L): larger = more votes, then lower linear index
+    int removed, stop;
+};
+
+__global__ void __launch_bounds__(512)
+hough_peel_kernel(const DevParams P, int S, const float* __restrict__ u, const float* __restrict__ v,
+                  const long long* __restrict__ offsets, int n_events, Candidate* __restrict__ cands, int* __restrict__ n_found,
+                  int* __restrict__ labels)
+{
+    HOUGH_DYNAMIC_SMEM(smem);
+    __shared__ PeelShared sh;
+    __shared__ unsigned long long wbest[16];
+    int* tile = reinterpret_cast<int*>(smem);  // [S][n_rho]
+    const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
+    const int half = P.F >= 1 ? (1 << (P.F - 1)) : 0;
+    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+        const long long g0 = offsets[e], g1 = offsets[e + 1];
+        __syncthreads();
+        if (g0 < 0 || g1 < g0 || (g1 - g0) > (long long)P.max_hits_per_event) {
+            if (tid == 0) { atomicOr(P.status, (g0 < 0 || g1 < g0) ? 2 : 1); n_found[e] = 0; }
+            if (g0 >= 0 && g1 >= g0) for (long long i = g0 + tid; i < g1; i += nthr) labels[i] = -1;
+            continue;
+        }
+        const int ne = (int)(g1 - g0);
+        for (int i = tid; i < ne; i += nthr) labels[g0 + i] = -1;
+        int n_tracks = 0;
+        while (n_tracks < P.K) {
+            __syncthreads();  // labels of the previous track are written
+            if (tid == 0) { sh.best = 0ull; sh.removed = 0; sh.stop = 0; }
+            for (int base = 0; base < P.n_theta; base += S) {
+                const int rows = min(S, P.n_theta - base);
+                for (int i = tid; i < rows * P.n_rho; i += nthr) tile[i] = 0;
+                __syncthreads();
+                // one thread per (remaining hit, theta row of the strip)
+                for (long long w = tid; w < (long long)ne * rows; w += nthr) {
+                    const int h = (int)(w / rows), tl = (int)(w - (long long)h * rows);
+                    if (labels[g0 + h] >= 0) continue;  // already on a track
+                    const float uf = __ldg(u + g0 + h), vf = __ldg(v + g0 + h);
+                    if (!(fabsf(uf) <= P.coord_max) || !(fabsf(vf) <= P.coord_max)) continue;
+                    const int uq = __float2int_rn(uf * P.hit_scale), vq = __float2int_rn(vf * P.hit_scale);
+                    const int a = uq * __ldg(P.Cq + base + tl) + (vq * __ldg(P.Sq + base + tl) + P.Oq);
+                    const int r = a >> P.F;
+                    if ((unsigned)r < (unsigned)P.n_rho && HB(P, tl * P.n_rho + r, S * P.n_rho, 320)) atomicAdd(&tile[tl * P.n_rho + r], 1);
+                }
+                __syncthreads();
+                unsigned long long best = 0ull;
+                for (int i = tid; i < rows * P.n_rho; i += nthr) {
+                    const unsigned c = (unsigned)tile[i];
+                    if (c) {
+                        const unsigned L = (unsigned)(base * P.n_rho + i);  // i = tl * n_rho + r
+                        const unsigned long long key = ((unsigned long long)c << 32) | (unsigned long long)(0xffffffffu - L);
+                        if (key > best) best = key;
+                    }
+                }
+#pragma unroll
+                for (int o = 16; o; o >>= 1) { const unsigned long long y = __shfl_xor_sync(0xffffffffu, best, o); if (y > best) best = y; }
+                if (lane == 0) wbest[warp] = best;
+                __syncthreads();
+                if (tid == 0) {
+                    unsigned long long b = sh.best;
+                    for (int k = 0; k < (nthr >> 5); ++k) if (wbest[k] > b) b = wbest[k];
+                    sh.best = b;
+                }
+                __syncthreads();  // the tile may be cleared again
+            }
+            const unsigned long long best = sh.best;
+            const int votes = (int)(best >> 32);
+            if (votes < P.T) break;  // block-uniform: nothing above the threshold is left
+            const unsigned L = 0xffffffffu - (unsigned)(best & 0xffffffffull);
+            const int tb = (int)(L / (unsigned)P.n_rho), rb = (int)(L - (unsigned)tb * P.n_rho);
+            const int Ct = __ldg(P.Cq + tb), St = __ldg(P.Sq + tb), Oc = P.Oq - (rb << P.F) - half;
+            int mine = 0;
+            for (int i = tid; i < ne; i += nthr) {
+                if (labels[g0 + i] >= 0) continue;
+                const float uf = __ldg(u + g0 + i), vf = __ldg(v + g0 + i);
+                if (!(fabsf(uf) <= P.coord_max) || !(fabsf(vf) <= P.coord_max)) continue;
+                const int uq = __float2int_rn(uf * P.hit_scale), vq = __float2int_rn(vf * P.hit_scale);
+                const int ev = uq * Ct + (vq * St + Oc);
+                if ((unsigned)abs(ev) <= (unsigned)P.Wq) { labels[g0 + i] = n_tracks; ++mine; }
+            }
+            if (mine) atomicAdd(&sh.removed, mine);
+            __syncthreads();
+            if (sh.removed == 0) break;  // a window narrower than half a bin missed every voter: no progress (B7)
+            if (tid == 0) {
+                const float th = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)tb), (double)P.n_theta);
+                const float rho = (float)__dadd_rn(P.rho_min, __dmul_rn((double)rb + 0.5, P.d_rho));
+                int4* dst = reinterpret_cast<int4*>(cands + (size_t)e * P.K + n_tracks);
+                dst[0] = make_int4(tb, rb, votes, n_tracks);
+                dst[1] = make_int4(0, __float_as_int(th), __float_as_int(rho), 0);
+            }
+            ++n_tracks;
+        }
+        if (tid == 0) n_found[e] = n_tracks;
+    }
+}
+
 }  // namespace hough

@@ -35,7 +35,7 @@ EXPORTS = ("hough_plan_create", "hough_plan_destroy", "hough_vote", "hough_find_
            "hough_run_host", "hough_run_host_chunked", "hough_plan_query", "hough_plan_status", "hough_plan_launch_count", "hough_plan_debug_counters",
            "hough_measure_smem_atomic_peak", "hough_strerror", "hough_last_cuda_error", "hough_version",
            "hough_refit_tracks", "hough_frontend_create", "hough_frontend_destroy", "hough_frontend_slice",
-           "hough_frontend_status")
+           "hough_frontend_status", "hough_find_tracks_peeloff")
 
 
 class hough_plan_desc_t(ctypes.Structure):
@@ -115,6 +115,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     L.hough_last_cuda_error.restype = ctypes.c_char_p
     L.hough_version.argtypes = []
     L.hough_refit_tracks.argtypes = [vp, vp, vp, vp, i32, vp, vp, ctypes.POINTER(hough_plane_geometry_t), vp, vp]
+    L.hough_find_tracks_peeloff.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp, vp]
     L.hough_frontend_create.argtypes = [ctypes.POINTER(hough_frontend_desc_t), ctypes.POINTER(vp)]
     L.hough_frontend_destroy.argtypes = [vp]
     L.hough_frontend_slice.argtypes = [vp, vp, vp, vp, vp, vp, i32, i64, vp, vp, vp, vp, i64, vp]
@@ -394,3 +395,17 @@ def hough_frontend_status(fe: FrontEnd, stream=None) -> int:
     s = stream if stream is not None else torch.cuda.current_stream(fe.device)
     _check(load_library().hough_frontend_status(fe.handle, ctypes.byref(out), ctypes.c_void_p(s.cuda_stream)), "hough_frontend_status")
     return out.value
+
+
+def hough_find_tracks_peeloff(plan: Plan, u: torch.Tensor, v: torch.Tensor, offsets: torch.Tensor, stream=None):
+    """The paper's one-track-at-a-time peak rule (variant).  -> (cands int32 [E, K, 8], n_found int32 [E], labels int32 [N])."""
+    E = _n_events(offsets)
+    cands = torch.zeros((E, plan.K, CANDIDATE_WORDS), dtype=torch.int32, device=plan.device)
+    n_found = torch.zeros(E, dtype=torch.int32, device=plan.device)
+    labels = torch.empty(max(u.numel(), 1), dtype=torch.int32, device=plan.device)
+    _check(load_library().hough_find_tracks_peeloff(plan.handle, _dev(plan, u, torch.float32, "u"), _dev(plan, v, torch.float32, "v"),
+                                                    _dev(plan, offsets, torch.int64, "offsets"), E,
+                                                    _dev(plan, cands, torch.int32, "cands"), _dev(plan, n_found, torch.int32, "n_found"),
+                                                    _dev(plan, labels, torch.int32, "labels"), _stream_ptr(plan, stream)),
+           "hough_find_tracks_peeloff")
+    return cands, n_found, labels[: u.numel()]

@@ -365,3 +365,39 @@ def test_frontend_feeds_the_hough_core():
         fits_equal(fits[e], fo_e)
         found += sum(1 for f in fo_e if f.flags & T.FIT_FOUND)
     assert found >= 3
+
+
+def peel_case(seed, n_tracks, n_noise):
+    rng = np.random.default_rng(seed)
+    us, vs = [], []
+    for _ in range(n_tracks):
+        uu, vv = synth.ideal_track(rng.uniform(-1, 1), rng.uniform(-100, 100))
+        keep = rng.random(48) > 0.1
+        us.append(uu[keep]); vs.append((vv + rng.normal(0, 0.1, 48).astype(np.float32))[keep])
+    us.append(rng.uniform(-94, 94, n_noise).astype(np.float32)); vs.append(rng.uniform(-194, 194, n_noise).astype(np.float32))
+    u, v = np.concatenate(us), np.concatenate(vs)
+    pm = rng.permutation(len(u))
+    return u[pm], v[pm]
+
+
+@pytest.mark.parametrize("grid,K,w_bins", [((64, 128), 8, 1.5), ((45, 300), 2, 1.0), ((90, 77), 6, 0.25)])
+def test_peeloff_variant(grid, K, w_bins):
+    """O13: the paper's own peak rule, one track at a time, against the step-by-step oracle (tracks in the order found, labels)."""
+    p = std_params(grid[0], grid[1], T=12, K=K, w_bins=w_bins)
+    us, vs, offs = [], [], [0]
+    for e, (nt, nn) in enumerate([(3, 12), (0, 0), (1, 40), (4, 5), (0, 25)]):
+        u, v = peel_case(50 + e, nt, nn) if nt + nn else (np.zeros(0, np.float32), np.zeros(0, np.float32))
+        us.append(u); vs.append(v); offs.append(offs[-1] + len(u))
+    u, v, offsets = np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64)
+    u[5] = np.nan                                                           # an invalid hit: never on a track
+    g = E.peeloff(p, u, v, offsets)
+    assert g["status"] == 0
+    for e in range(len(offsets) - 1):
+        a, z = int(offsets[e]), int(offsets[e + 1])
+        tracks, labels = T.peel_event(u[a:z], v[a:z], p)
+        assert int(g["n_found"][e]) == len(tracks)
+        got = [(int(c["theta_bin"]), int(c["rho_bin"]), int(c["votes"])) for c in g["cands"][e, :len(tracks)]]
+        assert got == tracks
+        assert [int(c["cluster_root"]) for c in g["cands"][e, :len(tracks)]] == list(range(len(tracks)))
+        np.testing.assert_array_equal(g["labels"][a:z], labels)
+    assert g["n_found"][0] >= (2 if w_bins >= 1.0 else 1) and g["labels"][5] == -1

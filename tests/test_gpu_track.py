@@ -150,3 +150,29 @@ def test_whole_chain_fills_to_fits():
         found += sum(1 for f in fo_e if f.flags & T.FIT_FOUND)
     assert found >= 60
     H.hough_plan_destroy(plan)
+
+
+@pytest.mark.parametrize("grid,K,w_bins", [((64, 128), 8, 1.5), ((180, 1000), 6, 2.0)])
+def test_peeloff_variant(grid, K, w_bins):
+    """O13 on the GPU against the step-by-step oracle: tracks in the order found, labels."""
+    from test_emulated_kernels import peel_case
+    p = D.Params(grid[0], grid[1], -256.0, 256.0, 256.0, 12, w_bins * 512.0 / grid[1], K)
+    us, vs, offs = [], [], [0]
+    for e, (nt, nn) in enumerate([(3, 12), (0, 0), (1, 40), (4, 5), (0, 25), (2, 0)] * 3):
+        u, v = peel_case(70 + e, nt, nn) if nt + nn else (np.zeros(0, np.float32), np.zeros(0, np.float32))
+        us.append(u); vs.append(v); offs.append(offs[-1] + len(u))
+    u, v, offsets = np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64)
+    E = len(offsets) - 1
+    plan = H.hough_plan_create(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.vote_threshold, p.assign_window,
+                               p.max_candidates, E, len(u), int(np.diff(offsets).max()))
+    cands, n_found, labels = H.hough_find_tracks_peeloff(plan, dev(u, np.float32), dev(v, np.float32), dev(offsets, np.int64))
+    torch.cuda.synchronize()
+    assert H.hough_plan_status(plan) == 0 and int(H.hough_plan_debug_counters(plan)[14]) == 0
+    gc, gn, gl = H.candidates_to_numpy(cands), n_found.cpu().numpy(), labels.cpu().numpy()
+    H.hough_plan_destroy(plan)
+    for e in range(E):
+        a, z = int(offsets[e]), int(offsets[e + 1])
+        tracks, lab = T.peel_event(u[a:z], v[a:z], p)
+        assert int(gn[e]) == len(tracks)
+        assert [(int(c["theta_bin"]), int(c["rho_bin"]), int(c["votes"])) for c in gc[e, :len(tracks)]] == tracks
+        np.testing.assert_array_equal(gl[a:z], lab)
