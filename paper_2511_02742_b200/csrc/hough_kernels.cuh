@@ -617,10 +617,14 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
 // One CTA per event at a time; the event's kept candidates become (C_q[t_s], S_q[t_s], O_q - r_s 2^F - 2^(F-1))
 // triples in shared memory; each thread owns hits and scans the triples (warp-uniform broadcast reads).
 
+// KEYED: the running arg-min is one packed key per hit, key = min(|e|, W_q + 1) * 2^kbits + slot with 2^kbits >= K, so that
+// "smaller |e|, then lower slot" is a single unsigned minimum (IABS + VIMNMX + VIADDMNMX on sm_100a: three ALU-pipe
+// instructions per residual instead of four); the host picks it when (W_q + 2) * 2^kbits fits 32 bits.
+template <bool KEYED>
 __global__ void __launch_bounds__(256)
 hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float* __restrict__ v,
                     const long long* __restrict__ offsets, int n_events, const Candidate* __restrict__ cands,
-                    const int* __restrict__ n_found, int* __restrict__ labels)
+                    const int* __restrict__ n_found, int* __restrict__ labels, int kbits, unsigned key_mul)
 {
     HOUGH_DYNAMIC_SMEM(smem);
     int4* trip = reinterpret_cast<int4*>(smem);  // [K]
@@ -635,7 +639,7 @@ hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float*
             const Candidate* c = cands + (size_t)e * P.K + s;
             const int t = c->theta_bin, r = c->rho_bin;
             const int half = P.F >= 1 ? (1 << (P.F - 1)) : 0;
-            trip[s] = make_int4(__ldg(P.Cq + t), __ldg(P.Sq + t), P.Oq - (r << P.F) - half, 0);
+            trip[s] = make_int4(__ldg(P.Cq + t), __ldg(P.Sq + t), P.Oq - (r << P.F) - half, s);
         }
         __syncthreads();
         // HPT hits per thread and trip: one broadcast load of a candidate triple serves HPT residuals.  best starts at
@@ -657,14 +661,34 @@ hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float*
                 best[j] = best0;
                 label[j] = -1;
             }
-#pragma unroll 2
-            for (int s = 0; s < nk; ++s) {
-                const int4 c = trip[s];
+            if (KEYED) {
+                // best0 = W_q + 1: an ineligible residual.  key_mul = 2^kbits arrives as a kernel parameter so that the key is
+                // ONE IMAD (multiply-add on the FMA pipe) and not a shift + add on the ALU pipe, which binds this loop
+                const unsigned clampv = best0, mul = key_mul;
 #pragma unroll
-                for (int j = 0; j < HPT; ++j) {
-                    const int ev = uq[j] * c.x + (vq[j] * c.y + c.z);
-                    const unsigned ae = (unsigned)abs(ev);
-                    if (ae < best[j]) { best[j] = ae; label[j] = s; }
+                for (int j = 0; j < HPT; ++j) best[j] = 0xffffffffu;
+#pragma unroll 2
+                for (int s = 0; s < nk; ++s) {
+                    const int4 c = trip[s];
+#pragma unroll
+                    for (int j = 0; j < HPT; ++j) {
+                        const int ev = uq[j] * c.x + (vq[j] * c.y + c.z);
+                        const unsigned ae = min((unsigned)abs(ev), clampv);
+                        best[j] = min(best[j], ae * mul + (unsigned)c.w);
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < HPT; ++j) label[j] = (best[j] >> kbits) < clampv ? (int)(best[j] & (mul - 1u)) : -1;
+            } else {
+#pragma unroll 2
+                for (int s = 0; s < nk; ++s) {
+                    const int4 c = trip[s];
+#pragma unroll
+                    for (int j = 0; j < HPT; ++j) {
+                        const int ev = uq[j] * c.x + (vq[j] * c.y + c.z);
+                        const unsigned ae = (unsigned)abs(ev);
+                        if (ae < best[j]) { best[j] = ae; label[j] = s; }
+                    }
                 }
             }
 #pragma unroll

@@ -595,10 +595,20 @@ int hough_assign_hits(hough_plan_t* p, const float* d_u, const float* d_v, const
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     HCK(cudaSetDevice(p->desc.device));
     const int grid = n_events < p->assign_ctas ? n_events : p->assign_ctas;
-    if ((size_t)p->P.K * 16 > 48 * 1024)
-        HCK(cudaFuncSetAttribute(hough::hough_assign_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, p->P.K * 16));
-    HOUGH_LAUNCH(hough::hough_assign_kernel, grid, 256, (size_t)p->P.K * 16, st, p->P, d_u, d_v, reinterpret_cast<const long long*>(d_offsets),
-                 n_events, reinterpret_cast<const Candidate*>(d_cands), d_n_found, d_labels);
+    int kbits = 0;
+    while ((1 << kbits) < p->P.K) ++kbits;
+    // one packed key (|e| clamped to W_q + 1, then the slot) per hit if it fits 32 bits; else the two-register arg-min
+    const bool keyed = ((unsigned long long)((unsigned)p->P.Wq + 2u) << kbits) <= 0xffffffffull;
+    const size_t smem = (size_t)p->P.K * 16;
+    if (keyed) {
+        if (smem > 48 * 1024) HCK(cudaFuncSetAttribute(hough::hough_assign_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        HOUGH_LAUNCH(hough::hough_assign_kernel<true>, grid, 256, smem, st, p->P, d_u, d_v, reinterpret_cast<const long long*>(d_offsets),
+                     n_events, reinterpret_cast<const Candidate*>(d_cands), d_n_found, d_labels, kbits, 1u << kbits);
+    } else {
+        if (smem > 48 * 1024) HCK(cudaFuncSetAttribute(hough::hough_assign_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        HOUGH_LAUNCH(hough::hough_assign_kernel<false>, grid, 256, smem, st, p->P, d_u, d_v, reinterpret_cast<const long long*>(d_offsets),
+                     n_events, reinterpret_cast<const Candidate*>(d_cands), d_n_found, d_labels, kbits, 1u << kbits);
+    }
     HCK(cudaGetLastError());
     p->launches += 1;
     return HOUGH_OK;
