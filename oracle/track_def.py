@@ -29,6 +29,13 @@ Readings (B1-B8):
   B6  plane (vane) index of a hit = nearest plane: floor((u - origin) / pitch + 1/2), counted only inside [0, n_planes);
       "continuous five" = a run of >= min_run consecutive plane indices that each hold >= 1 assigned hit; with wrap the
       planes form a ring (the 40 vanes of the detector).
+  B8  two-stage (coarse -> fine) Hough, PAPER.md L124 / Fig. 5 ("a coarse-binning histogram followed by a fine-binning
+      histogram"; no further detail in the paper): the coarse grid merges c_theta x c_rho fine bins; a coarse row T votes at
+      the fine theta row in its middle, t_T = min(T c_theta + c_theta // 2, n_theta - 1), into coarse bin r_fine // c_rho;
+      coarse peaks = strict local maxima >= T of the coarse histogram under the same total order, the best K kept; every kept
+      coarse peak (T, R) opens a fine patch of the coarse bins T-1..T+1 x R-1..R+1 (clipped to the grid), filled exactly as
+      O3 does; its candidate is the patch's maximum under (count, -L) if count >= T; duplicates are merged and the result is
+      ranked like O6.  cluster_root = own slot, cluster_nbins = 0 (no clustering in this variant).
   B7  peel-off: the global maximum under the total order (count, -L); stop when its count < T or after K tracks; its hits are
       those within the assignment window of its bin-centre line; they are removed from the hit set and the histogram is
       refilled from the remaining hits (equivalently: their votes are subtracted); a maximum none of whose hits lies inside
@@ -248,3 +255,43 @@ def peel_event(u: Sequence, v: Sequence, p: D.Params) -> Tuple[List[Tuple[int, i
             break
         tracks.append((tb, rb, int(acc[tb, rb])))
     return tracks, labels
+
+
+# ----------------------------------------------------------------------------- O14 two-stage (coarse -> fine) Hough
+def two_stage_event(u: Sequence, v: Sequence, p: D.Params, c_theta: int, c_rho: int) -> Tuple[List[Tuple[int, int, int]], int]:
+    """B8.  Returns ([(theta_bin, rho_bin, votes)] ranked by (votes desc, linear index asc), n_found)."""
+    k = D.constants(p)
+    two_f = 2 ** k.F
+    nT, nR = -(-p.n_theta // c_theta), -(-p.n_rho // c_rho)
+    hits = [h for h in (D.quantise_hit(u[i], v[i], p, k) for i in range(len(u))) if h[0]]
+    coarse = np.zeros((nT, nR), np.int64)
+    for _, uq, vq in hits:
+        for T in range(nT):
+            t = min(T * c_theta + c_theta // 2, p.n_theta - 1)
+            r = D.fixed_point_rho(uq, vq, t, k) // two_f
+            if 0 <= r < p.n_rho:
+                coarse[T, r // c_rho] += 1
+    pc = D.Params(nT, nR, p.rho_min, p.rho_max, p.coord_max, p.vote_threshold, p.assign_window, p.max_candidates, p.hit_frac_bits, k.F)
+    cpk = D.peaks(coarse, pc)
+    cpk.sort(key=lambda b: (-int(coarse[b]), b[0] * nR + b[1]))
+    found = {}
+    for (T, R) in cpk[: p.max_candidates]:
+        t0, t1 = max(0, (T - 1) * c_theta), min(p.n_theta, (T + 2) * c_theta)
+        r0, r1 = max(0, (R - 1) * c_rho), min(p.n_rho, (R + 2) * c_rho)
+        patch = np.zeros((t1 - t0, r1 - r0), np.int64)
+        for _, uq, vq in hits:
+            for t in range(t0, t1):
+                r = D.fixed_point_rho(uq, vq, t, k) // two_f
+                if r0 <= r < r1:
+                    patch[t - t0, r - r0] += 1
+        best = None
+        for t in range(t0, t1):
+            for r in range(r0, r1):
+                key = (int(patch[t - t0, r - r0]), -(t * p.n_rho + r))
+                if best is None or key > best:
+                    best = key
+        if best is not None and best[0] >= p.vote_threshold:
+            L = -best[1]
+            found[L] = best[0]
+    ranked = sorted(found.items(), key=lambda kv: (-kv[1], kv[0]))
+    return [(L // p.n_rho, L % p.n_rho, c) for L, c in ranked], len(ranked)

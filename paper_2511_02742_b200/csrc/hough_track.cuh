@@ -125,7 +125,7 @@ fe_scatter_kernel(const FrontParams FP, const float* __restrict__ z, const long 
     const unsigned lt = (1u << lane) - 1u;
     for (int f = warp; f < n_fills; f += n_warps) {
         const long long a = fill_offsets[f], b = fill_offsets[f + 1];
-        long long* cur = FP.cursor + (long long)f * FP.windows_per_fill;
+        volatile long long* cur = FP.cursor + (long long)f * FP.windows_per_fill;  // written by lane 0, read by all lanes of this warp
         for (long long i0 = a; i0 < b; i0 += 32) {
             const long long i = i0 + lane;
             int nxt = 0x7fffffff, last = -1;

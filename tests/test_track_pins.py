@@ -221,3 +221,41 @@ def test_peel_off_finds_ideal_tracks_one_by_one():
     acc = D.vote_event(u, v, p)
     cands, _ = D.find_clusters_event(acc, p)
     assert (tracks[0][0], tracks[0][1], tracks[0][2]) == (cands[0].theta_bin, cands[0].rho_bin, cands[0].votes)
+
+
+# ----------------------------------------------------------------------------- O14 two-stage (coarse -> fine) Hough
+def test_two_stage_with_unit_factors_reproduces_patch_maxima_of_the_exact_histogram():
+    """c_theta = c_rho = 1: the coarse histogram IS the exact one, so every exact peak is a coarse peak and the maximum of its
+    3 x 3 patch is the peak itself: the two-stage list equals the one-pass list (O4, O6) without the cluster fields."""
+    p = std_params(64, 64, T=10, K=16)
+    u, v = peel_case_like(21)
+    two, n2 = T.two_stage_event(u, v, p, 1, 1)
+    acc = D.vote_event(u, v, p)
+    cands, n1 = D.find_clusters_event(acc, p)
+    assert n1 <= p.max_candidates
+    assert two == [(c.theta_bin, c.rho_bin, c.votes) for c in cands] and n2 == n1
+
+
+def test_two_stage_candidates_carry_exact_counts_and_find_the_tracks():
+    p = std_params(180, 256, T=24, K=16)
+    u, v = peel_case_like(22, n_tracks=3, n_noise=15)
+    acc = D.vote_event(u, v, p)
+    for ct, cr in ((4, 4), (3, 8), (6, 2)):
+        two, n2 = T.two_stage_event(u, v, p, ct, cr)
+        assert n2 == len(two) >= 2                                           # (close tracks can share one coarse peak)
+        for t, r, c in two:
+            assert acc[t, r] == c                                            # fine patches are filled exactly as O3 does
+        assert two == sorted(two, key=lambda x: (-x[2], x[0] * p.n_rho + x[1]))
+        # the global maximum of the exact histogram is found whenever its coarse neighbourhood held a coarse peak
+        tb, rb = np.unravel_index(np.argmax(acc), acc.shape)
+        assert two[0][2] == acc[tb, rb]
+
+
+def peel_case_like(seed, n_tracks=2, n_noise=8):
+    rng = np.random.default_rng(seed)
+    us, vs = [], []
+    for _ in range(n_tracks):
+        uu, vv = synth.ideal_track(rng.uniform(-1, 1), rng.uniform(-100, 100))
+        us.append(uu); vs.append(vv + rng.normal(0, 0.1, 48).astype(np.float32))
+    us.append(rng.uniform(-94, 94, n_noise).astype(np.float32)); vs.append(rng.uniform(-194, 194, n_noise).astype(np.float32))
+    return np.concatenate(us), np.concatenate(vs)
