@@ -185,6 +185,18 @@ int hough_find_tracks_peeloff(hough_plan_t* plan, const float* d_u, const float*
                               int32_t n_events, hough_candidate_t* d_cands, int32_t* d_n_found, int32_t* d_labels,
                               void* stream);
 
+/* Variant: the paper's two-stage histogram.  PAPER.md L124, Fig. 5: "we perform the Hough
+ * transformation into two stages: a coarse-binning histogram followed by a fine-binning histogram ... staying within the GPU's
+ * shared memory constraints".  Per event: a coarse histogram whose bins merge coarse_theta x coarse_rho bins of the plan's grid
+ * (coarse row T votes at the fine theta row in its middle); its strict local maxima >= T, the best K of them; for each a fine
+ * patch of the 3 x 3 coarse bins around it, filled exactly; the patch maximum is a candidate if it has >= T votes; duplicates
+ * are merged, records ranked by (votes descending, t * n_rho + r ascending), cluster_root = slot, cluster_nbins = 0.  An
+ * approximation of hough_find_clusters by design: a track whose coarse bin is not a coarse local maximum is missed.
+ * HOUGH_ERANGE if the coarse histogram and its lists exceed 200 KB of shared memory (choose coarser factors).
+ *   d_cands, d_n_found   as for hough_find_clusters (usable by hough_assign_hits / hough_refit_tracks) */
+int hough_find_two_stage(hough_plan_t* plan, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events,
+                         int32_t coarse_theta, int32_t coarse_rho, hough_candidate_t* d_cands, int32_t* d_n_found, void* stream);
+
 /* Front end: RecoHits (x, y, z, t) of a batch of fills -> one event per time window, in the (phi, z) plane.
  * "the reconstructed hit points are divided into overlapping time windows of 10 ns, with a sliding step of
  * 5 ns.  Within each time window, the spatial coordinates (x, y, z) of the hits are transformed into the (phi, z) space".

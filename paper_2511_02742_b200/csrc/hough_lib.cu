@@ -826,6 +826,39 @@ int hough_find_tracks_peeloff(hough_plan_t* p, const float* d_u, const float* d_
     return HOUGH_OK;
 }
 
+// ---------------------------------------------------------------- variant: two-stage (coarse -> fine) Hough (hough_track.cuh)
+
+int hough_find_two_stage(hough_plan_t* p, const float* d_u, const float* d_v, const int64_t* d_offsets, int32_t n_events,
+                         int32_t coarse_theta, int32_t coarse_rho, hough_candidate_t* d_cands, int32_t* d_n_found, void* stream)
+{
+    int rc = check_common(p, d_u, d_v, d_offsets, n_events);
+    if (rc) return rc;
+    if (!d_cands || !d_n_found || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_n_found & 3)) return HOUGH_EINVAL;
+    if (coarse_theta < 1 || coarse_rho < 1 || coarse_theta > p->desc.n_theta || coarse_rho > p->desc.n_rho) return HOUGH_EINVAL;
+    hough::TwoStageParams Q;
+    Q.c_theta = coarse_theta; Q.c_rho = coarse_rho;
+    Q.nT = (p->desc.n_theta + coarse_theta - 1) / coarse_theta;
+    Q.nR = (p->desc.n_rho + coarse_rho - 1) / coarse_rho;
+    Q.cp_cap = ((Q.nT + 1) / 2) * ((Q.nR + 1) / 2);
+    size_t o = align_up((size_t)Q.nT * Q.nR * 4, 16);
+    Q.off_patch = (int)o;  o = align_up(o + (size_t)9 * coarse_theta * coarse_rho * 4, 16);
+    Q.off_cpeaks = (int)o; o = align_up(o + (size_t)Q.cp_cap * 8, 16);
+    Q.off_ckept = (int)o;  o = align_up(o + (size_t)p->P.K * 8, 16);
+    Q.off_fkeys = (int)o;  o = align_up(o + (size_t)p->P.K * 8, 16);
+    if (o > 200u * 1024u) return HOUGH_ERANGE;  // the coarse histogram and its lists must fit shared memory: coarser factors
+    if (n_events == 0) return HOUGH_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    HCK(cudaSetDevice(p->desc.device));
+    if (o > 48 * 1024) HCK(cudaFuncSetAttribute(hough::hough_two_stage_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)o));
+    const int cap = p->info.n_sm * 2;
+    const int grid = n_events < cap ? n_events : cap;
+    HOUGH_LAUNCH(hough::hough_two_stage_kernel, grid, 512, o, st, p->P, Q, d_u, d_v, reinterpret_cast<const long long*>(d_offsets), n_events,
+                 reinterpret_cast<Candidate*>(d_cands), d_n_found);
+    HCK(cudaGetLastError());
+    p->launches += 1;
+    return HOUGH_OK;
+}
+
 // ---------------------------------------------------------------- front end: time slicing + phi (hough_track.cuh)
 
 struct hough_frontend {

@@ -349,4 +349,168 @@ hough_peel_kernel(const DevParams P, int S, const float* __restrict__ u, const f
     }
 }
 
+// ---------------------------------------------------------------- variant: two-stage (coarse -> fine) Hough (O14, reading B8)
+//
+// The paper's own answer to the shared-memory limit (Fig. 5: "a coarse-binning histogram followed by a
+// fine-binning histogram").  One CTA per event: coarse histogram (c_theta x c_rho fine bins per coarse bin, one theta row per
+// coarse row) -> coarse local maxima -> best K -> per kept coarse peak a fine patch of 3 x 3 coarse bins filled exactly,
+// its maximum is the candidate; duplicates merged, ranked by (votes desc, linear index asc).
+struct TwoStageParams {
+    int c_theta, c_rho, nT, nR;   // coarse factors and coarse grid
+    int cp_cap;                   // capacity of the coarse-peak list: ceil(nT / 2) * ceil(nR / 2) (no two strict maxima touch)
+    int off_patch, off_cpeaks, off_ckept, off_fkeys;  // byte offsets into dynamic shared memory (the coarse tile starts at 0)
+};
+
+struct TwoStageShared {
+    int n_cp, n_f;
+    unsigned long long best;
+};
+
+__device__ __forceinline__ bool ts_hit(const DevParams& P, const float* __restrict__ u, const float* __restrict__ v, long long i, int& uq, int& vq)
+{
+    const float uf = __ldg(u + i), vf = __ldg(v + i);
+    if (!(fabsf(uf) <= P.coord_max) || !(fabsf(vf) <= P.coord_max)) return false;
+    uq = __float2int_rn(uf * P.hit_scale);
+    vq = __float2int_rn(vf * P.hit_scale);
+    return true;
+}
+
+__global__ void __launch_bounds__(512)
+hough_two_stage_kernel(const DevParams P, const TwoStageParams Q, const float* __restrict__ u, const float* __restrict__ v,
+                       const long long* __restrict__ offsets, int n_events, Candidate* __restrict__ cands, int* __restrict__ n_found)
+{
+    HOUGH_DYNAMIC_SMEM(smem);
+    __shared__ TwoStageShared sh;
+    __shared__ unsigned long long wbest[16];
+    int* coarse = reinterpret_cast<int*>(smem);                                                    // [nT][nR]
+    int* patch = reinterpret_cast<int*>(smem + Q.off_patch);                                       // [3 c_theta][3 c_rho]
+    unsigned long long* cpeaks = reinterpret_cast<unsigned long long*>(smem + Q.off_cpeaks);       // [cp_cap]
+    unsigned long long* ckept = reinterpret_cast<unsigned long long*>(smem + Q.off_ckept);         // [K]
+    unsigned long long* fkeys = reinterpret_cast<unsigned long long*>(smem + Q.off_fkeys);         // [K]
+    const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
+    const int n_cbins = Q.nT * Q.nR;
+    for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
+        const long long g0 = offsets[e], g1 = offsets[e + 1];
+        __syncthreads();
+        if (g0 < 0 || g1 < g0 || (g1 - g0) > (long long)P.max_hits_per_event) {
+            if (tid == 0) { atomicOr(P.status, (g0 < 0 || g1 < g0) ? 2 : 1); n_found[e] = 0; }
+            continue;
+        }
+        const int ne = (int)(g1 - g0);
+        if (tid == 0) { sh.n_cp = 0; sh.n_f = 0; }
+        for (int i = tid; i < n_cbins; i += nthr) coarse[i] = 0;
+        __syncthreads();
+        // ---- stage 1: coarse histogram, one thread per (hit, coarse row)
+        for (long long w = tid; w < (long long)ne * Q.nT; w += nthr) {
+            const int h = (int)(w / Q.nT), T = (int)(w - (long long)h * Q.nT);
+            int uq, vq;
+            if (!ts_hit(P, u, v, g0 + h, uq, vq)) continue;
+            const int t = min(T * Q.c_theta + Q.c_theta / 2, P.n_theta - 1);
+            const int r = (uq * __ldg(P.Cq + t) + (vq * __ldg(P.Sq + t) + P.Oq)) >> P.F;
+            if ((unsigned)r < (unsigned)P.n_rho && HB(P, T * Q.nR + r / Q.c_rho, n_cbins, 330)) atomicAdd(&coarse[T * Q.nR + r / Q.c_rho], 1);
+        }
+        __syncthreads();
+        // ---- coarse peaks: strict local maxima >= T under (count, -index)
+        for (int i = tid; i < n_cbins; i += nthr) {
+            const int c = coarse[i];
+            if (c < P.T) continue;
+            const int T = i / Q.nR, R = i - T * Q.nR;
+            bool pk = true;
+            for (int dT = -1; dT <= 1 && pk; ++dT)
+                for (int dR = -1; dR <= 1; ++dR) {
+                    if (!dT && !dR) continue;
+                    const int TT = T + dT, RR = R + dR;
+                    if (TT < 0 || TT >= Q.nT || RR < 0 || RR >= Q.nR) continue;
+                    const int j = TT * Q.nR + RR, cj = coarse[j];
+                    if (cj > c || (cj == c && j < i)) { pk = false; break; }
+                }
+            if (pk) {
+                const int k = atomicAdd(&sh.n_cp, 1);
+                if (HB(P, k, Q.cp_cap, 331)) cpeaks[k] = ((unsigned long long)(unsigned)c << 32) | (unsigned long long)(0xffffffffu - (unsigned)i);
+            }
+        }
+        __syncthreads();
+        const int n_cp = min(sh.n_cp, Q.cp_cap), n_ck = min(n_cp, P.K);
+        for (int i = tid; i < n_cp; i += nthr) {  // rank by counting (keys are unique): the K largest keys, best first
+            const unsigned long long key = cpeaks[i];
+            int rank = 0;
+            for (int j = 0; j < n_cp; ++j) rank += (cpeaks[j] > key);
+            if (rank < P.K) ckept[rank] = key;
+        }
+        __syncthreads();
+        // ---- stage 2: one exact fine patch per kept coarse peak
+        const int PR = 3 * Q.c_rho;
+        for (int s = 0; s < n_ck; ++s) {
+            const unsigned ci = 0xffffffffu - (unsigned)(ckept[s] & 0xffffffffull);
+            const int T = (int)(ci / (unsigned)Q.nR), R = (int)(ci - (unsigned)T * Q.nR);
+            const int t0 = max(0, (T - 1) * Q.c_theta), t1 = min(P.n_theta, (T + 2) * Q.c_theta);
+            const int r0 = max(0, (R - 1) * Q.c_rho), r1 = min(P.n_rho, (R + 2) * Q.c_rho);
+            const int rows = t1 - t0;
+            for (int i = tid; i < 3 * Q.c_theta * PR; i += nthr) patch[i] = 0;
+            __syncthreads();
+            for (long long w = tid; w < (long long)ne * rows; w += nthr) {
+                const int h = (int)(w / rows), t = t0 + (int)(w - (long long)h * rows);
+                int uq, vq;
+                if (!ts_hit(P, u, v, g0 + h, uq, vq)) continue;
+                const int r = (uq * __ldg(P.Cq + t) + (vq * __ldg(P.Sq + t) + P.Oq)) >> P.F;
+                if (r >= r0 && r < r1 && HB(P, (t - t0) * PR + (r - r0), 3 * Q.c_theta * PR, 332)) atomicAdd(&patch[(t - t0) * PR + (r - r0)], 1);
+            }
+            __syncthreads();
+            unsigned long long best = 0ull;
+            for (int i = tid; i < rows * PR; i += nthr) {
+                const int tl = i / PR, rl = i - tl * PR;
+                const unsigned c = (unsigned)patch[i];
+                if (c && r0 + rl < r1) {
+                    const unsigned L = (unsigned)((t0 + tl) * P.n_rho + r0 + rl);
+                    const unsigned long long key = ((unsigned long long)c << 32) | (unsigned long long)(0xffffffffu - L);
+                    if (key > best) best = key;
+                }
+            }
+#pragma unroll
+            for (int o = 16; o; o >>= 1) { const unsigned long long y = __shfl_xor_sync(0xffffffffu, best, o); if (y > best) best = y; }
+            if (lane == 0) wbest[warp] = best;
+            __syncthreads();
+            if (tid == 0) {
+                unsigned long long b = 0ull;
+                for (int k = 0; k < (nthr >> 5); ++k) if (wbest[k] > b) b = wbest[k];
+                if ((int)(b >> 32) >= P.T) fkeys[sh.n_f++] = b;
+            }
+            __syncthreads();  // the patch may be cleared again
+        }
+        // ---- merge duplicates, rank (votes desc, linear index asc), write the records
+        const int n_f = sh.n_f;
+        for (int i = tid; i < n_f; i += nthr) {
+            const unsigned long long key = fkeys[i];
+            bool dup = false;
+            for (int j = 0; j < i; ++j) dup |= (fkeys[j] == key);
+            if (dup) continue;
+            int rank = 0;
+            for (int j = 0; j < n_f; ++j) {
+                if (fkeys[j] > key) {  // count every distinct larger key once: at its first occurrence
+                    bool first = true;
+                    for (int q = 0; q < j; ++q) first &= (fkeys[q] != fkeys[j]);
+                    rank += first;
+                }
+            }
+            const unsigned L = 0xffffffffu - (unsigned)(key & 0xffffffffull);
+            const int t = (int)(L / (unsigned)P.n_rho), r = (int)(L - (unsigned)t * P.n_rho);
+            const float th = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)t), (double)P.n_theta);
+            const float rho = (float)__dadd_rn(P.rho_min, __dmul_rn((double)r + 0.5, P.d_rho));
+            int4* dst = reinterpret_cast<int4*>(cands + (size_t)e * P.K + rank);
+            dst[0] = make_int4(t, r, (int)(key >> 32), rank);
+            dst[1] = make_int4(0, __float_as_int(th), __float_as_int(rho), 0);
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int distinct = 0;
+            for (int i = 0; i < n_f; ++i) {
+                bool dup = false;
+                for (int j = 0; j < i; ++j) dup |= (fkeys[j] == fkeys[i]);
+                distinct += !dup;
+            }
+            n_found[e] = distinct;
+        }
+    }
+}
+
 }  // namespace hough

@@ -35,7 +35,7 @@ EXPORTS = ("hough_plan_create", "hough_plan_destroy", "hough_vote", "hough_find_
            "hough_run_host", "hough_run_host_chunked", "hough_plan_query", "hough_plan_status", "hough_plan_launch_count", "hough_plan_debug_counters",
            "hough_measure_smem_atomic_peak", "hough_strerror", "hough_last_cuda_error", "hough_version",
            "hough_refit_tracks", "hough_frontend_create", "hough_frontend_destroy", "hough_frontend_slice",
-           "hough_frontend_status", "hough_find_tracks_peeloff")
+           "hough_frontend_status", "hough_find_tracks_peeloff", "hough_find_two_stage")
 
 
 class hough_plan_desc_t(ctypes.Structure):
@@ -116,6 +116,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     L.hough_version.argtypes = []
     L.hough_refit_tracks.argtypes = [vp, vp, vp, vp, i32, vp, vp, ctypes.POINTER(hough_plane_geometry_t), vp, vp]
     L.hough_find_tracks_peeloff.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp, vp]
+    L.hough_find_two_stage.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp]
     L.hough_frontend_create.argtypes = [ctypes.POINTER(hough_frontend_desc_t), ctypes.POINTER(vp)]
     L.hough_frontend_destroy.argtypes = [vp]
     L.hough_frontend_slice.argtypes = [vp, vp, vp, vp, vp, vp, i32, i64, vp, vp, vp, vp, i64, vp]
@@ -407,5 +408,18 @@ def hough_find_tracks_peeloff(plan: Plan, u: torch.Tensor, v: torch.Tensor, offs
                                                     _dev(plan, offsets, torch.int64, "offsets"), E,
                                                     _dev(plan, cands, torch.int32, "cands"), _dev(plan, n_found, torch.int32, "n_found"),
                                                     _dev(plan, labels, torch.int32, "labels"), _stream_ptr(plan, stream)),
-           "hough_find_tracks_peeloff")
+           "hough_find_tracks_peeloff", "hough_find_two_stage")
     return cands, n_found, labels[: u.numel()]
+
+
+def hough_find_two_stage(plan: Plan, u: torch.Tensor, v: torch.Tensor, offsets: torch.Tensor, coarse_theta: int, coarse_rho: int,
+                         stream=None):
+    """The paper's coarse -> fine two-stage histogram (variant).  -> (cands int32 [E, K, 8], n_found int32 [E])."""
+    E = _n_events(offsets)
+    cands = torch.zeros((E, plan.K, CANDIDATE_WORDS), dtype=torch.int32, device=plan.device)
+    n_found = torch.zeros(E, dtype=torch.int32, device=plan.device)
+    _check(load_library().hough_find_two_stage(plan.handle, _dev(plan, u, torch.float32, "u"), _dev(plan, v, torch.float32, "v"),
+                                               _dev(plan, offsets, torch.int64, "offsets"), E, coarse_theta, coarse_rho,
+                                               _dev(plan, cands, torch.int32, "cands"), _dev(plan, n_found, torch.int32, "n_found"),
+                                               _stream_ptr(plan, stream)), "hough_find_two_stage")
+    return cands, n_found

@@ -259,3 +259,27 @@ def peeloff(p, u, v, offsets, max_hpe=None):
     assert L.cuda_emu_violations() == 0, L.cuda_emu_first_violation().decode()
     assert int(dbg[14]) == 0, f"index check failed at site {int(dbg[13])}"
     return dict(cands=cands.view.copy(), n_found=n_found.view.copy(), labels=labels.view[: len(u)].copy(), status=st.value)
+
+
+def two_stage(p, u, v, offsets, c_theta, c_rho):
+    """hough_find_two_stage on the emulated device -> dict(cands, n_found, rc)."""
+    L = lib()
+    L.cuda_emu_reset_violations()
+    vp, i32 = ctypes.c_void_p, ctypes.c_int32
+    L.hough_find_two_stage.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, vp]
+    E = len(offsets) - 1
+    hpe = int(np.diff(offsets).max()) if E > 0 and len(u) else 0
+    d = Desc(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.hit_frac_bits, p.acc_frac_bits, p.vote_threshold,
+             p.assign_window, p.max_candidates, HOUGH_I32, max(1, E), max(0, len(u)), max(hpe, 1), 0, 0)
+    h = ctypes.c_void_p()
+    assert L.hough_plan_create(ctypes.byref(d), ctypes.byref(h)) == 0
+    du, dv, do = DevBuf(np.asarray(u, np.float32)), DevBuf(np.asarray(v, np.float32)), DevBuf(np.asarray(offsets, np.int64))
+    cands = DevBuf(np.zeros((E, p.max_candidates), CAND_DTYPE))
+    n_found = DevBuf(np.full(E, -5, np.int32))
+    rc = L.hough_find_two_stage(h, du.ptr, dv.ptr, do.ptr, E, c_theta, c_rho, cands.ptr, n_found.ptr, None)
+    dbg = np.zeros(16, np.uint64)
+    L.hough_plan_debug_counters(h, dbg.ctypes.data, None)
+    L.hough_plan_destroy(h)
+    assert L.cuda_emu_violations() == 0, L.cuda_emu_first_violation().decode()
+    assert int(dbg[14]) == 0, f"index check failed at site {int(dbg[13])}"
+    return dict(cands=cands.view.copy(), n_found=n_found.view.copy(), rc=rc)

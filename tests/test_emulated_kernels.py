@@ -401,3 +401,32 @@ def test_peeloff_variant(grid, K, w_bins):
         assert [int(c["cluster_root"]) for c in g["cands"][e, :len(tracks)]] == list(range(len(tracks)))
         np.testing.assert_array_equal(g["labels"][a:z], labels)
     assert g["n_found"][0] >= (2 if w_bins >= 1.0 else 1) and g["labels"][5] == -1
+
+
+@pytest.mark.parametrize("grid,factors,K", [((180, 256), (4, 4), 16), ((180, 1000), (4, 8), 8), ((64, 64), (1, 1), 16), ((90, 100), (7, 3), 4)])
+def test_two_stage_variant(grid, factors, K):
+    """O14: the paper's coarse -> fine two-stage histogram against the step-by-step oracle (ranked candidates, counts)."""
+    p = D.Params(grid[0], grid[1], -256.0, 256.0, 256.0, 12, 512.0 / grid[1], K)
+    us, vs, offs = [], [], [0]
+    for e, (nt, nn) in enumerate([(3, 12), (0, 0), (1, 40), (5, 30), (0, 25)]):
+        u, v = peel_case(60 + e, nt, nn) if nt + nn else (np.zeros(0, np.float32), np.zeros(0, np.float32))
+        us.append(u); vs.append(v); offs.append(offs[-1] + len(u))
+    u, v, offsets = np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64)
+    g = E.two_stage(p, u, v, offsets, *factors)
+    assert g["rc"] == 0
+    total = 0
+    for e in range(len(offsets) - 1):
+        a, z = int(offsets[e]), int(offsets[e + 1])
+        want, n = T.two_stage_event(u[a:z], v[a:z], p, *factors)
+        assert int(g["n_found"][e]) == n
+        got = [(int(c["theta_bin"]), int(c["rho_bin"]), int(c["votes"])) for c in g["cands"][e, :n]]
+        assert got == want
+        assert [int(c["cluster_root"]) for c in g["cands"][e, :n]] == list(range(n))
+        total += n
+    assert total >= 4
+
+
+def test_two_stage_rejects_a_coarse_grid_that_does_not_fit_shared_memory():
+    p = std_params(512, 512, T=20, K=16)
+    z = np.zeros(4, np.float32)
+    assert E.two_stage(p, z, z, np.array([0, 4], np.int64), 1, 1)["rc"] == -2

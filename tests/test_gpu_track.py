@@ -176,3 +176,28 @@ def test_peeloff_variant(grid, K, w_bins):
         assert int(gn[e]) == len(tracks)
         assert [(int(c["theta_bin"]), int(c["rho_bin"]), int(c["votes"])) for c in gc[e, :len(tracks)]] == tracks
         np.testing.assert_array_equal(gl[a:z], lab)
+
+
+@pytest.mark.parametrize("grid,factors,K", [((180, 256), (4, 4), 16), ((180, 1000), (4, 8), 8)])
+def test_two_stage_variant(grid, factors, K):
+    """O14 on the GPU against the step-by-step oracle: ranked candidates with their exact counts."""
+    from test_emulated_kernels import peel_case
+    p = D.Params(grid[0], grid[1], -256.0, 256.0, 256.0, 12, 512.0 / grid[1], K)
+    us, vs, offs = [], [], [0]
+    for e, (nt, nn) in enumerate([(3, 12), (0, 0), (1, 40), (5, 30), (0, 25), (2, 3)] * 4):
+        u, v = peel_case(80 + e, nt, nn) if nt + nn else (np.zeros(0, np.float32), np.zeros(0, np.float32))
+        us.append(u); vs.append(v); offs.append(offs[-1] + len(u))
+    u, v, offsets = np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64)
+    E = len(offsets) - 1
+    plan = H.hough_plan_create(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.vote_threshold, p.assign_window,
+                               p.max_candidates, E, len(u), int(np.diff(offsets).max()))
+    cands, n_found = H.hough_find_two_stage(plan, dev(u, np.float32), dev(v, np.float32), dev(offsets, np.int64), *factors)
+    torch.cuda.synchronize()
+    assert H.hough_plan_status(plan) == 0 and int(H.hough_plan_debug_counters(plan)[14]) == 0
+    gc, gn = H.candidates_to_numpy(cands), n_found.cpu().numpy()
+    H.hough_plan_destroy(plan)
+    for e in range(E):
+        a, z = int(offsets[e]), int(offsets[e + 1])
+        want, n = T.two_stage_event(u[a:z], v[a:z], p, *factors)
+        assert int(gn[e]) == n
+        assert [(int(c["theta_bin"]), int(c["rho_bin"]), int(c["votes"])) for c in gc[e, :n]] == want
