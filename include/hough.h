@@ -67,7 +67,7 @@ typedef struct {
     double coord_max;             /* a hit is valid iff finite and |u|, |v| <= coord_max                    */
     int32_t hit_frac_bits;        /* H: hits are rounded to multiples of 2^-H (ties to even); < 0 -> 6      */
     int32_t acc_frac_bits;        /* F: fraction bits of the fixed-point rho bin coordinate; < 0 -> largest
-                                     F <= 24 that keeps every intermediate inside int32                    */
+                                     F <= 24 that keeps every intermediate (votes and bin centres) in int32 */
     int32_t vote_threshold;       /* T >= 1: a bin is "on" iff its count >= T                               */
     double assign_window;         /* w >= 0, in rho units: a hit may join a candidate iff its distance to
                                      the candidate's bin-centre line is <= w                               */

@@ -88,9 +88,11 @@ def _llround(x: float) -> int:
 
 def default_frac_bits(p: Params) -> int:
     """O2: largest F <= 24 with span * 2^F <= 2^31 - 1,
-    span = sqrt(2) coord_max / d_rho + max(|rho_min|, |rho_max|) / d_rho + 2."""
+    span = max(sqrt(2) coord_max / d_rho + max(|rho_min|, |rho_max|) / d_rho + 2, n_rho + 1): every intermediate of O3 AND the
+    bin centres r 2^F + 2^(F-1) of O7 (r < n_rho) stay inside int32."""
     d_rho = (p.rho_max - p.rho_min) / p.n_rho
     span = math.sqrt(2.0) * p.coord_max / d_rho + max(abs(p.rho_min), abs(p.rho_max)) / d_rho + 2.0
+    span = max(span, float(p.n_rho + 1))
     F = 24
     while F > 0 and span * float(2 ** F) > float(INT32_MAX):
         F -= 1

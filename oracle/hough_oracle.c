@@ -58,6 +58,7 @@ int ho_default_frac_bits(const ho_params_t* p)
     double a = fabs(p->rho_min), b = fabs(p->rho_max);
     double span = sqrt(2.0) * p->coord_max / d_rho + (a > b ? a : b) / d_rho + 2.0;
     int F = 24;
+    if (span < (double)p->n_rho + 1.0) span = (double)p->n_rho + 1.0;  /* bin centres r 2^F + 2^(F-1), r < n_rho (O7) */
     while (F > 0 && span * pow2i(F) > 2147483647.0) --F;
     return F;
 }

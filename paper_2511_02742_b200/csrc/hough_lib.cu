@@ -229,7 +229,8 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     int F = d->acc_frac_bits;
     if (F < 0) {
         const double amin = fabs(d->rho_min), amax = fabs(d->rho_max);
-        const double span = sqrt(2.0) * d->coord_max / d_rho + (amin > amax ? amin : amax) / d_rho + 2.0;
+        double span = sqrt(2.0) * d->coord_max / d_rho + (amin > amax ? amin : amax) / d_rho + 2.0;
+        if (span < (double)d->n_rho + 1.0) span = (double)d->n_rho + 1.0;  // the bin centres r 2^F + 2^(F-1) of the assignment fit too
         F = 24;
         while (F > 0 && span * ldexp(1.0, F) > 2147483647.0) --F;
     }

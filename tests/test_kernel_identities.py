@@ -33,7 +33,7 @@ def test_vote_address_folding(n_theta, n_rho, G):
     kk = int(np.log2(row_bytes))
     sh = k.F - kk
     assert sh >= 0
-    tile_base = 1024  # dynamic shared memory window offset: a multiple of the row size, below 4096
+    tile_base = 1024  # dynamic shared memory window offset: a multiple of the row size, below 4096 (the kernel checks both at entry)
     assert ((4096 << sh) + (n_rho << k.F)) <= 0xFFFFFFFF  # the plan's admission test for the fast path
     rng = np.random.default_rng(7)
     lim = int(p.coord_max * (1 << k.H))

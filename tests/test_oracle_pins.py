@@ -139,6 +139,16 @@ def test_p1b_offset_and_window_round_half_away(impl):
         assert Oq == int(oq) and Wq == int(wq)
 
 
+def test_p1b_default_frac_bits_keeps_the_bin_centres_in_int32(impl):
+    """A rho range much wider than the hits (n_rho + 1 > the O3 span): F must shrink until (n_rho + 1) 2^F fits int32, so that the
+    bin centres of O7 do.  1025 * 2^20 < 2^31 - 1 < 1025 * 2^21."""
+    p = D.Params(16, 1024, -1.5, 1.5, 1.0, 2, 3.0 / 1024, 4, 6, -1)
+    H, F, Oq, Wq, Cq, Sq = impl.constants(p)
+    assert F == 20 and (p.n_rho + 1) * 2 ** F <= 2 ** 31 - 1 < (p.n_rho + 1) * 2 ** (F + 1)
+    assert Oq == 512 * 2 ** 20 and Wq == 2 ** 20
+    # the configs are unaffected (their O3 span exceeds n_rho + 1): F = 23 / 22 / 21 / 20 as before (test_p1_frac_bits...)
+
+
 # ----------------------------------------------------------------------------- P2 table CRC
 def test_p2_table_crc32(impl):
     for n_theta, crc in read_golden_table("table_crc32.txt"):
