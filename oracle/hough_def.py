@@ -53,6 +53,12 @@ class Params:
     max_candidates: int           # K
     hit_frac_bits: int = 6        # H
     acc_frac_bits: int = -1       # F; < 0 -> default formula
+    theta_min: float = 0.0        # theta window [theta_min, theta_max) in radians; the paper's is [0, pi)
+    theta_max: float = math.pi
+
+    def theta_of(self, t: int) -> float:
+        """theta_t = theta_min + (theta_max - theta_min) t / n_theta (left bin edge); for the default window pi t / n_theta."""
+        return self.theta_min + (self.theta_max - self.theta_min) * t / self.n_theta
 
 
 @dataclass(frozen=True)
@@ -100,13 +106,14 @@ def default_frac_bits(p: Params) -> int:
 
 
 def constants(p: Params) -> Constants:
-    """O2.  theta_t = pi t / n_theta (left bin edge, theta in [0, pi));  tables by formula in double."""
+    """O2.  theta_t = theta_min + (theta_max - theta_min) t / n_theta (left bin edge; the paper's window [0, pi) gives
+    pi t / n_theta, bit for bit);  tables by formula in double."""
     H = p.hit_frac_bits
     F = p.acc_frac_bits if p.acc_frac_bits >= 0 else default_frac_bits(p)
     d_rho = (p.rho_max - p.rho_min) / p.n_rho
     M = float(2 ** (F - H)) / d_rho if F >= H else 1.0 / (float(2 ** (H - F)) * d_rho)
-    Cq = tuple(_llround(math.cos(math.pi * t / p.n_theta) * M) for t in range(p.n_theta))
-    Sq = tuple(_llround(math.sin(math.pi * t / p.n_theta) * M) for t in range(p.n_theta))
+    Cq = tuple(_llround(math.cos(p.theta_of(t)) * M) for t in range(p.n_theta))
+    Sq = tuple(_llround(math.sin(p.theta_of(t)) * M) for t in range(p.n_theta))
     Oq = _llround(-p.rho_min * float(2 ** F) / d_rho)
     Wq = _llround(p.assign_window * float(2 ** F) / d_rho)
     return Constants(H, F, d_rho, M, Cq, Sq, Oq, Wq)
@@ -230,7 +237,7 @@ def find_clusters_event(acc: np.ndarray, p: Params) -> Tuple[List[Candidate], in
         root_bin, n_bins = comps[labels[t, r]]
         # the root out-ranks every peak of its component, so it is kept whenever one of them is
         out.append(Candidate(t, r, int(acc[t, r]), slot_of[root_bin], n_bins,
-                             np.float32(math.pi * t / p.n_theta), np.float32(p.rho_min + (r + 0.5) * d_rho)))
+                             np.float32(p.theta_of(t)), np.float32(p.rho_min + (r + 0.5) * d_rho)))
     return out, n_found
 
 

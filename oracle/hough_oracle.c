@@ -35,6 +35,7 @@ typedef struct {
     int32_t max_candidates;
     int32_t hit_frac_bits;
     int32_t acc_frac_bits; /* < 0: default */
+    double theta_min, theta_max; /* theta window in radians; (0, 0) = the paper's [0, pi) */
 } ho_params_t;
 
 typedef struct { /* 32 bytes, the record layout the public ABI documents */
@@ -49,6 +50,14 @@ typedef struct { /* 32 bytes, the record layout the public ABI documents */
 #define HO_EARG (-3)
 
 static const double HO_PI = 3.14159265358979323846;
+
+/* theta_t = theta_min + (theta_max - theta_min) t / n_theta; a window of (0, 0) means the paper's [0, pi),
+ * for which this is pi t / n_theta bit for bit (x + 0.0 == x). */
+static double ho_theta(const ho_params_t* p, int t)
+{
+    const double lo = p->theta_min, hi = (p->theta_min == 0.0 && p->theta_max == 0.0) ? HO_PI : p->theta_max;
+    return lo + (hi - lo) * t / p->n_theta;
+}
 
 static double pow2i(int e) { return ldexp(1.0, e); }
 
@@ -72,7 +81,7 @@ int ho_constants(const ho_params_t* p, int64_t* Cq, int64_t* Sq, int64_t* scal)
     double d_rho = (p->rho_max - p->rho_min) / p->n_rho;
     double M = pow2i(F - H) / d_rho;
     for (int t = 0; t < p->n_theta; ++t) {
-        double th = HO_PI * t / p->n_theta;
+        double th = ho_theta(p, t);
         Cq[t] = llround(cos(th) * M);
         Sq[t] = llround(sin(th) * M);
     }
@@ -214,7 +223,7 @@ int ho_find_clusters_event(const ho_params_t* p, const int32_t* acc, ho_cand_t* 
         cands[s].votes = pk[s].votes;
         cands[s].cluster_root = root_slot;
         cands[s].cluster_nbins = comp_size[c];
-        cands[s].theta = (float)(HO_PI * t / p->n_theta);
+        cands[s].theta = (float)ho_theta(p, t);
         cands[s].rho = (float)(p->rho_min + (r + 0.5) * d_rho);
         cands[s].reserved = 0;
     }

@@ -149,6 +149,35 @@ def test_p1b_default_frac_bits_keeps_the_bin_centres_in_int32(impl):
     # the configs are unaffected (their O3 span exceeds n_rho + 1): F = 23 / 22 / 21 / 20 as before (test_p1_frac_bits...)
 
 
+def test_p1c_theta_window(impl):
+    """Restricted theta window: theta_t = theta_min + (theta_max - theta_min) t / n_theta.  Closed forms at
+    the window's start, agreement with the rows of the full grid that sample the same angles, and the ideal-track peak (P5)."""
+    from dataclasses import replace
+    full = std_params(512, 256)
+    win = replace(std_params(256, 256), theta_min=math.pi / 4, theta_max=3 * math.pi / 4)
+    H, F, Oq, Wq, Cf, Sf = impl.constants(full)
+    Hw, Fw, Oqw, Wqw, Cw, Sw = impl.constants(win)
+    assert (Hw, Fw, Oqw, Wqw) == (H, F, Oq, Wq)
+    assert Cw[0] == Sw[0] == 23170 and Cw[128] == 0 and Sw[128] == 32768          # 45 degrees: M / sqrt(2); 90 degrees: (0, M)
+    assert np.abs(Cw - Cf[128:384]).max() <= 1 and np.abs(Sw - Sf[128:384]).max() <= 1   # same angles, last-bit rounding of theta only
+    assert (Cw == Cf[128:384]).mean() > 0.9
+    quarter = replace(std_params(64, 256), theta_min=math.pi / 2, theta_max=math.pi)
+    _, _, _, _, Cq, Sq = impl.constants(quarter)
+    assert Cq[0] == 0 and Sq[0] == 32768 and Cq[32] == -23170                         # 90 and 135 degrees
+    # P5 in the window: a noiseless track through the centre of bin (t*, r*) of the windowed grid
+    t_star, r_star = 70, 150
+    th = math.pi / 4 + (math.pi / 2) * t_star / 256
+    m, c = -1.0 / math.tan(th), (-256.0 + (r_star + 0.5) * 2.0) / math.sin(th)
+    uu, vv = synth.ideal_track(m, c)
+    acc = np.asarray(impl.vote(uu, vv, win))
+    assert acc[t_star, r_star] == 48 == acc.max()
+    cands, nf = impl.clusters(acc, win)
+    c0 = cands[0]
+    tb = c0.theta_bin if hasattr(c0, "theta_bin") else c0["theta_bin"]
+    thf = c0.theta if hasattr(c0, "theta") else c0["theta"]
+    assert acc[int(tb)].max() == 48 and abs(float(thf) - (math.pi / 4 + (math.pi / 2) * int(tb) / 256)) < 1e-6
+
+
 # ----------------------------------------------------------------------------- P2 table CRC
 def test_p2_table_crc32(impl):
     for n_theta, crc in read_golden_table("table_crc32.txt"):
