@@ -59,7 +59,7 @@ enum { HOUGH_FLAG_GENERAL_ONLY = 1, HOUGH_FLAG_SMALL_LISTS = 2 };
 typedef struct hough_plan hough_plan_t;           /* opaque; created and destroyed by the library */
 
 /* The (theta, rho) grid, thresholds and capacities of one plan.
- * theta always spans [0, pi): bin t stands for theta_t = pi t / n_theta (left edge; "0 to 180 deg").
+ * theta spans [0, pi) unless a window is given: bin t stands for theta_t = pi t / n_theta (left edge; "0 to 180 deg").
  * rho spans the half-open range [rho_min, rho_max) in n_rho equal bins (histogram semantics). */
 typedef struct {
     int32_t n_theta, n_rho;       /* >= 1; n_theta * n_rho <= 2^22                                          */
@@ -78,6 +78,9 @@ typedef struct {
     int32_t max_hits_per_event;   /* capacity: hits in one event (HOUGH_U16 needs <= 65535)                 */
     int32_t flags;                /* 0 or HOUGH_FLAG_* bits                                                 */
     int32_t device;               /* CUDA device ordinal                                                    */
+    double theta_min, theta_max;  /* theta window in radians, bin t stands for theta_min + (theta_max - theta_min)
+                                     t / n_theta; both 0 -> the paper's [0, pi); a narrower window
+                                     spends the theta bins where the tracks are (slopes within +-1: [pi/4, 3pi/4)) */
 } hough_plan_desc_t;
 
 /* One track candidate: a local maximum of the event's accumulator.  32 bytes, little endian. */

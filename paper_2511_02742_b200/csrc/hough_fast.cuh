@@ -663,7 +663,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             if (!HB(P, rs, n_kept, 158)) rs = 0;
             int t, r;
             split_L(P, L, t, r);
-            const float th = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)t), (double)P.n_theta);
+            const float th = theta_of_bin(P, t);
             const float rho = (float)__dadd_rn(P.rho_min, __dmul_rn((double)r + 0.5, P.d_rho));
             int4* dst = reinterpret_cast<int4*>(cands + (size_t)e * P.K + s);
             dst[0] = make_int4(t, r, (int)c, rs);

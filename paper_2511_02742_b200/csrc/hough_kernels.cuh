@@ -65,6 +65,7 @@ struct DevParams {
     int HB, PCAP;                            // capacity of the staged-hit buffer / the in-smem peak list
     int max_hits_per_event;
     double rho_min, d_rho;
+    double theta_min, theta_span;  // theta_t = theta_min + theta_span t / n_theta
     const int* Cq;  // [n_strips * S], zero padded
     const int* Sq;
     int off_hits, off_halo, off_peaks, off_kept, off_kroot, off_hist;  // byte offsets into dynamic smem
@@ -98,6 +99,12 @@ struct Candidate {  // mirrors hough_candidate_t
     float theta, rho;
     int reserved;
 };
+
+// S6: theta of bin t, the oracle's sequence of double operations (for the default window theta_min = 0, theta_span = pi)
+__device__ __forceinline__ float theta_of_bin(const DevParams& P, int t)
+{
+    return (float)__dadd_rn(P.theta_min, __ddiv_rn(__dmul_rn(P.theta_span, (double)t), (double)P.n_theta));
+}
 
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -595,7 +602,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
             cd.votes = (int)c;
             cd.cluster_root = rs;
             cd.cluster_nbins = (int)__ldcg(csize + root);
-            cd.theta = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)cd.theta_bin), (double)P.n_theta);
+            cd.theta = theta_of_bin(P, cd.theta_bin);
             cd.rho = (float)__dadd_rn(P.rho_min, __dmul_rn((double)cd.rho_bin + 0.5, P.d_rho));
             cd.reserved = 0;
             int4* dst = reinterpret_cast<int4*>(cands + (size_t)e * P.K + s);

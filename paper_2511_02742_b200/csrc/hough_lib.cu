@@ -219,6 +219,10 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     if (d->count_dtype != HOUGH_I32 && d->count_dtype != HOUGH_U16) return HOUGH_EINVAL;
     if (d->max_events < 1 || d->max_hits < 0 || d->max_hits_per_event < 0 || d->device < 0) return HOUGH_EINVAL;
     if (d->flags & ~(HOUGH_FLAG_GENERAL_ONLY | HOUGH_FLAG_SMALL_LISTS)) return HOUGH_EINVAL;
+    // theta window: (0, 0) = the paper's [0, pi)
+    const bool th_default = d->theta_min == 0.0 && d->theta_max == 0.0;
+    const double th_lo = d->theta_min, th_hi = th_default ? 3.14159265358979323846 : d->theta_max;
+    if (!isfinite(th_lo) || !isfinite(th_hi) || !(th_hi > th_lo) || th_hi - th_lo > 6.283185307179586) return HOUGH_EINVAL;
     if (d->count_dtype == HOUGH_U16 && d->max_hits_per_event > 65535) return HOUGH_ERANGE;  // a bin gets <= 1 vote per hit
     if ((int64_t)d->n_theta * d->n_rho > (1ll << hough::kLBits)) return HOUGH_ERANGE;
     const int H = d->hit_frac_bits < 0 ? 6 : d->hit_frac_bits;
@@ -250,7 +254,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     p->h_sin.resize(d->n_theta);
     long long max_cs = 0;
     for (int t = 0; t < d->n_theta; ++t) {
-        const double th = 3.14159265358979323846 * t / d->n_theta;
+        const double th = th_lo + (th_hi - th_lo) * t / d->n_theta;  // [0, pi): pi t / n_theta bit for bit
         const long long c = llround(cos(th) * M), s = llround(sin(th) * M);
         p->h_cos[t] = (int32_t)c;
         p->h_sin[t] = (int32_t)s;
@@ -437,6 +441,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     P.HB = HB; P.PCAP = PCAP;
     P.max_hits_per_event = d->max_hits_per_event;
     P.rho_min = d->rho_min; P.d_rho = d_rho;
+    P.theta_min = th_lo; P.theta_span = th_hi - th_lo;
     P.Cq = p->d_cos; P.Sq = p->d_sin;
     P.off_hits = lay.off_hits; P.off_halo = lay.off_halo; P.off_peaks = lay.off_peaks;
     P.off_kept = lay.off_kept; P.off_kroot = lay.off_kroot; P.off_hist = lay.off_hist;

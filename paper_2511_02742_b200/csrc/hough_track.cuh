@@ -337,7 +337,7 @@ hough_peel_kernel(const DevParams P, int S, const float* __restrict__ u, const f
             __syncthreads();
             if (sh.removed == 0) break;  // a window narrower than half a bin missed every voter: no progress (B7)
             if (tid == 0) {
-                const float th = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)tb), (double)P.n_theta);
+                const float th = theta_of_bin(P, tb);
                 const float rho = (float)__dadd_rn(P.rho_min, __dmul_rn((double)rb + 0.5, P.d_rho));
                 int4* dst = reinterpret_cast<int4*>(cands + (size_t)e * P.K + n_tracks);
                 dst[0] = make_int4(tb, rb, votes, n_tracks);
@@ -494,7 +494,7 @@ hough_two_stage_kernel(const DevParams P, const TwoStageParams Q, const float* _
             }
             const unsigned L = 0xffffffffu - (unsigned)(key & 0xffffffffull);
             const int t = (int)(L / (unsigned)P.n_rho), r = (int)(L - (unsigned)t * P.n_rho);
-            const float th = (float)__ddiv_rn(__dmul_rn(3.14159265358979323846, (double)t), (double)P.n_theta);
+            const float th = theta_of_bin(P, t);
             const float rho = (float)__dadd_rn(P.rho_min, __dmul_rn((double)r + 0.5, P.d_rho));
             int4* dst = reinterpret_cast<int4*>(cands + (size_t)e * P.K + rank);
             dst[0] = make_int4(t, r, (int)(key >> 32), rank);

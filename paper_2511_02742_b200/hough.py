@@ -44,7 +44,7 @@ class hough_plan_desc_t(ctypes.Structure):
                 ("acc_frac_bits", ctypes.c_int32), ("vote_threshold", ctypes.c_int32), ("assign_window", ctypes.c_double),
                 ("max_candidates", ctypes.c_int32), ("count_dtype", ctypes.c_int32), ("max_events", ctypes.c_int32),
                 ("max_hits", ctypes.c_int64), ("max_hits_per_event", ctypes.c_int32), ("flags", ctypes.c_int32),
-                ("device", ctypes.c_int32)]
+                ("device", ctypes.c_int32), ("theta_min", ctypes.c_double), ("theta_max", ctypes.c_double)]
 
 
 class hough_plan_info_t(ctypes.Structure):
@@ -152,10 +152,11 @@ class Plan:
 def hough_plan_create(n_theta: int, n_rho: int, rho_min: float, rho_max: float, coord_max: float, vote_threshold: int,
                       assign_window: float, max_candidates: int, max_events: int, max_hits: int, max_hits_per_event: int,
                       count_dtype: int = HOUGH_I32, hit_frac_bits: int = -1, acc_frac_bits: int = -1, device: int = 0,
-                      flags: int = 0) -> Plan:
+                      flags: int = 0, theta_min: float = 0.0, theta_max: float = 0.0) -> Plan:
     L = load_library()
     d = hough_plan_desc_t(n_theta, n_rho, rho_min, rho_max, coord_max, hit_frac_bits, acc_frac_bits, vote_threshold,
-                          assign_window, max_candidates, count_dtype, max_events, max_hits, max_hits_per_event, flags, device)
+                          assign_window, max_candidates, count_dtype, max_events, max_hits, max_hits_per_event, flags, device,
+                          theta_min, theta_max)
     h = ctypes.c_void_p()
     _check(L.hough_plan_create(ctypes.byref(d), ctypes.byref(h)), "hough_plan_create")
     return Plan(h.value, d)

@@ -26,7 +26,7 @@ class Desc(ctypes.Structure):
                 ("acc_frac_bits", ctypes.c_int32), ("vote_threshold", ctypes.c_int32), ("assign_window", ctypes.c_double),
                 ("max_candidates", ctypes.c_int32), ("count_dtype", ctypes.c_int32), ("max_events", ctypes.c_int32),
                 ("max_hits", ctypes.c_int64), ("max_hits_per_event", ctypes.c_int32), ("flags", ctypes.c_int32),
-                ("device", ctypes.c_int32)]
+                ("device", ctypes.c_int32), ("theta_min", ctypes.c_double), ("theta_max", ctypes.c_double)]
 
 
 INFO_FIELDS = ("hit_frac_bits", "acc_frac_bits", "rho_offset_q", "assign_window_q", "strip_rows", "n_strips", "counter_bytes",
@@ -73,6 +73,13 @@ def configure(seed: int = 0, preempt_per_1024: int = 0, smem_window: int = 1024)
     lib().cuda_emu_configure(seed, preempt_per_1024, smem_window)
 
 
+def theta_window(p):
+    """(theta_min, theta_max) of the descriptor for oracle parameters: the default window is spelled (0, 0)."""
+    import math
+    lo, hi = getattr(p, "theta_min", 0.0), getattr(p, "theta_max", math.pi)
+    return (0.0, 0.0) if (lo == 0.0 and hi == math.pi) else (lo, hi)
+
+
 class DevBuf:
     """A "device" buffer of the emulated runtime is plain host memory; inputs are copied so that alignment is the caller's."""
 
@@ -98,7 +105,7 @@ def run(p, u, v, offsets, count_dtype=HOUGH_I32, want_acc=True, max_hpe=None, fl
     hpe = int(np.diff(offsets).max()) if E > 0 and len(u) else 0
     d = Desc(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.hit_frac_bits, p.acc_frac_bits, p.vote_threshold,
              p.assign_window, p.max_candidates, count_dtype, max(1, E), max(0, len(u)), max(hpe, 1) if max_hpe is None else max_hpe,
-             flags, 0)
+             flags, 0, *theta_window(p))
     h = ctypes.c_void_p()
     rc = L.hough_plan_create(ctypes.byref(d), ctypes.byref(h))
     assert rc == 0, f"hough_plan_create -> {rc}"

@@ -430,3 +430,21 @@ def test_two_stage_rejects_a_coarse_grid_that_does_not_fit_shared_memory():
     p = std_params(512, 512, T=20, K=16)
     z = np.zeros(4, np.float32)
     assert E.two_stage(p, z, z, np.array([0, 4], np.int64), 1, 1)["rc"] == -2
+
+
+def test_restricted_theta_window():
+    """theta window [pi/4, 3pi/4) -- the slopes within +-1 of the generator's tracks -- at the same angular
+    resolution with half the rows (and half the votes); fast and general kernel against the oracle, records incl. the fp32 theta."""
+    import math
+    from dataclasses import replace
+    wl = synth.workload(3)
+    b = synth.generate(wl, 0, 3)
+    p = replace(params_of(wl), n_theta=256, theta_min=math.pi / 4, theta_max=3 * math.pi / 4)
+    o = oracle_run(p, b.u, b.v, b.offsets)
+    for flags in (0, E.FLAG_GENERAL_ONLY):
+        g = E.run(p, b.u, b.v, b.offsets, E.HOUGH_U16, flags=flags)
+        assert_same(g, o, p)
+        for e in range(3):
+            k = min(int(o["n_found"][e]), p.max_candidates)
+            assert g["cands"][e, :k].tobytes() == o["cands"][e, :k].tobytes()
+    assert (o["cands"]["theta"][0, :8] >= math.pi / 4 - 1e-6).all() and (o["cands"]["theta"][0, :8] < 3 * math.pi / 4).all()

@@ -20,7 +20,8 @@ INT_FIELDS = ("theta_bin", "rho_bin", "votes", "cluster_root", "cluster_nbins", 
 def make_plan(p: D.Params, n_events, n_hits, max_hpe, count_dtype=H.HOUGH_I32, flags=0):
     return H.hough_plan_create(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.vote_threshold, p.assign_window,
                                p.max_candidates, max(1, n_events), max(0, n_hits), max_hpe, count_dtype,
-                               p.hit_frac_bits, p.acc_frac_bits, 0, flags)
+                               p.hit_frac_bits, p.acc_frac_bits, 0, flags,
+                               *((0.0, 0.0) if (p.theta_min == 0.0 and p.theta_max == np.pi) else (p.theta_min, p.theta_max)))
 
 
 def gpu_run(p: D.Params, u, v, offsets, count_dtype=H.HOUGH_I32, want_acc=True, max_hpe=None, flags=0, want_vote=True):
@@ -400,3 +401,18 @@ def test_bad_arguments_are_rejected_not_crashed():
         H.hough_find_clusters(plan, torch.zeros(8, device="cuda"), torch.zeros(8, device="cuda"), off_big)
     assert ei.value.status == H.HOUGH_ERANGE
     H.hough_plan_destroy(plan)
+
+
+def test_restricted_theta_window():
+    """theta window [pi/4, 3pi/4) at the resolution of cfg3 with half the rows; records incl. the fp32 theta."""
+    from dataclasses import replace
+    wl = synth.workload(3)
+    b = synth.generate(wl, 0, 200)
+    p = replace(params_of(wl), n_theta=256, theta_min=np.pi / 4, theta_max=3 * np.pi / 4)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    for flags in (0, H.HOUGH_FLAG_GENERAL_ONLY):
+        g = gpu_run(p, b.u, b.v, b.offsets, H.HOUGH_U16, want_acc=False, flags=flags)
+        assert_same(g, o, p)
+        for e in range(200):
+            k = min(int(o["n_found"][e]), p.max_candidates)
+            assert g["cands"][e, :k].tobytes() == o["cands"][e, :k].tobytes()
