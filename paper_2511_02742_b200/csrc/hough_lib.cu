@@ -160,10 +160,13 @@ static cudaError_t dispatch_fast(const hough_plan* p, const float* u, const floa
 {
 #define HOUGH_FCASE(G_, T_, B_)                                                                   \
     if (p->f_G == G_ && p->f_maxt == T_ && p->f_minb == B_) return launch_fast<G_, T_, B_>(p, u, v, off, n_events, cands, n_found, st);
-    HOUGH_FCASE(1, 768, 2) HOUGH_FCASE(2, 768, 2) HOUGH_FCASE(4, 768, 2)
-    HOUGH_FCASE(1, 1024, 2) HOUGH_FCASE(2, 1024, 2) HOUGH_FCASE(4, 1024, 2)
+    // the shapes hough_plan_create can choose (its preference list); the tuning build adds the ones experiments asked for
     HOUGH_FCASE(1, 1024, 1) HOUGH_FCASE(2, 1024, 1) HOUGH_FCASE(4, 1024, 1)
+    HOUGH_FCASE(1, 768, 2) HOUGH_FCASE(2, 768, 2) HOUGH_FCASE(4, 768, 2)
+#ifdef HOUGH_TUNING
+    HOUGH_FCASE(1, 1024, 2) HOUGH_FCASE(2, 1024, 2) HOUGH_FCASE(4, 1024, 2)
     HOUGH_FCASE(1, 512, 3) HOUGH_FCASE(2, 512, 3)
+#endif
 #undef HOUGH_FCASE
     return cudaErrorInvalidValue;
 }

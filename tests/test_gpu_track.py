@@ -97,6 +97,7 @@ def test_refit_tracks(cfg, n_events, geom):
 
 def check_refit(cfg, n_events, geom):
     wl = synth.workload(cfg)
+    wl = wl.with_events(max(wl.n_events, n_events))
     b = synth.generate(wl, 0, n_events)
     p = params_of(wl)
     o = C.run_batch(b.u, b.v, b.offsets, p)

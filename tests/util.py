@@ -53,6 +53,7 @@ def mixed_batch(cfg, n_events, seed, long_hits=0):
     """Generator events with special ones interleaved: empty events, an event whose hits all coincide 1100 times (a bin count
     above 1023: the fast kernel must hand it over), all-invalid events, and optionally one event of `long_hits` hits."""
     wl = synth.workload(cfg)
+    wl = wl.with_events(max(wl.n_events, n_events))      # more events than the config lists: further chunks of the same stream
     b = synth.generate(wl, 0, n_events)
     rng = np.random.default_rng(seed)
     us, vs, offs, kinds = [], [], [0], []
