@@ -75,7 +75,10 @@ typedef struct {
     int32_t count_dtype;          /* HOUGH_I32 or HOUGH_U16                                                 */
     int32_t max_events;           /* capacity: events per call                                              */
     int64_t max_hits;             /* capacity: hits per call                                                */
-    int32_t max_hits_per_event;   /* capacity: hits in one event (HOUGH_U16 needs <= 65535)                 */
+    int32_t max_hits_per_event;   /* capacity: hits in one event (HOUGH_U16 needs <= 65535).  Size it to the
+                                     workload: the fast kernel stages this many hits in shared memory, at the
+                                     cost of its other per-event lists (events that overflow those are still
+                                     correct, but recomputed by the slower general kernel)                  */
     int32_t flags;                /* 0 or HOUGH_FLAG_* bits                                                 */
     int32_t device;               /* CUDA device ordinal                                                    */
     double theta_min, theta_max;  /* theta window in radians, bin t stands for theta_min + (theta_max - theta_min)

@@ -25,7 +25,7 @@ def build(force: bool = False) -> str:
     # -DHOUGH_BOUNDS: the kernels' own index checks are compiled in as well (a failed check is reported, not performed)
     cmd = ["g++", "-std=c++17", "-O2", "-g", "-fPIC", "-shared", "-ffp-contract=off", "-fno-strict-aliasing", "-DHOUGH_EMU", "-DHOUGH_BOUNDS",
            "-Wall", "-Wno-unused-function", "-Wno-unused-variable", "-Wno-unknown-pragmas", "-Wno-sign-compare",
-           "-I", _HERE, "-x", "c++", os.path.join(_CSRC, "hough_lib.cu"), os.path.join(_HERE, "cuda_emu.cpp"), "-o", tmp]
+           "-I", _HERE, "-x", "c++", os.path.join(_CSRC, "hough_lib.cu"), os.path.join(_HERE, "cuda_emu.cpp"), "-o", tmp, "-pthread"]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

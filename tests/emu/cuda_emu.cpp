@@ -5,7 +5,11 @@
 #include <sys/mman.h>
 #include <unistd.h>
 
+#include <algorithm>
+#include <atomic>
 #include <map>
+#include <mutex>
+#include <thread>
 #include <vector>
 
 // Context switch (x86-64 System V): callee-saved registers go on the old stack, stack pointers are swapped.
@@ -56,25 +60,31 @@ struct Warp {
     unsigned gen[32];  // per lane: bumped when the collective the lane waits in completes
 };
 
-Fiber* g_cur = nullptr;
-unsigned char* g_smem = nullptr;
-unsigned g_smem_bytes = 0;
+// Per OS thread ("worker"): the CTA it is running.  With one worker (the default) the CTAs of a grid run one after another;
+// with several (cuda_emu_set_workers) each worker takes the next CTA of the grid, so that persistent CTAs really share the
+// work counter, the deferred list and their per-CTA scratch slabs, and global atomics are real atomics.
+thread_local Fiber* g_cur = nullptr;
+thread_local unsigned char* g_smem = nullptr;
+thread_local unsigned g_smem_bytes = 0;
 unsigned g_smem_window = 1024;
 dim3 g_block_dim, g_grid_dim;
 long long g_violations = 0;
 
-static uint3 g_block_idx;
-static void* g_sched_sp = nullptr;
+static thread_local uint3 g_block_idx;
+static thread_local void* g_sched_sp = nullptr;
 static const std::function<void()>* g_body = nullptr;
-static std::vector<Fiber> g_fibers;
-static std::vector<Warp> g_warps;
-static std::vector<unsigned char*> g_stacks;
-static std::vector<int> g_ready;  // runnable fibers that are not running
-static int g_n_barrier = 0, g_n_done = 0;
+static thread_local std::vector<Fiber> g_fibers;
+static thread_local std::vector<Warp> g_warps;
+static thread_local std::vector<unsigned char*> g_stacks;
+static thread_local std::vector<int> g_ready;  // runnable fibers that are not running
+static thread_local int g_n_barrier = 0, g_n_done = 0;
 static const size_t kStackBytes = 256 * 1024;
-static unsigned long long g_rng = 0x9E3779B97F4A7C15ull;
+static unsigned long long g_seed = 0x9E3779B97F4A7C15ull;
+static thread_local unsigned long long g_rng = 0x9E3779B97F4A7C15ull;
 static int g_preempt_per_1024 = 0;  // chance (in 1/1024) that an atomic / cache-bypassing access yields first
+static int g_workers = 1;
 static char g_first_violation[256] = "";
+static std::mutex g_mutex;
 
 static unsigned rnd()
 {
@@ -87,6 +97,7 @@ uint3 cur_block_idx() { return g_block_idx; }
 
 void violation(const char* what, unsigned long long a, unsigned long long lim)
 {
+    std::lock_guard<std::mutex> lock(g_mutex);
     if (g_violations == 0) {
         snprintf(g_first_violation, sizeof g_first_violation, "%s (value %llu, limit %llu; block %u thread %d)", what, a, lim,
                  g_block_idx.x, g_cur ? g_cur->tid : -1);
@@ -211,66 +222,86 @@ void dev_free(void* p)
     g_allocs.erase(it);
 }
 
-void launch(dim3 grid, dim3 block, size_t smem_bytes, const std::function<void()>& body)
+static void run_cta(unsigned b, int nthr, unsigned char* smem, size_t smem_bytes)
 {
-    const int nthr = (int)block.x;
-    g_block_dim = block;
-    g_grid_dim = grid;
-    g_body = &body;
     while ((int)g_stacks.size() < nthr) {
         unsigned char* st = static_cast<unsigned char*>(mmap(nullptr, kStackBytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0));
         if (st == MAP_FAILED) { fprintf(stderr, "cuda_emu: out of memory for fiber stacks\n"); abort(); }
         mprotect(st, 4096, PROT_NONE);
         g_stacks.push_back(st);
     }
-    size_t smem_map = 0; void* smem_base = nullptr;
-    unsigned char* smem = static_cast<unsigned char*>(guarded(smem_bytes ? smem_bytes : 16, &smem_map, &smem_base));
-    for (unsigned b = 0; b < grid.x; ++b) {
-        g_block_idx = uint3{b, 0, 0};
-        g_smem = smem;
-        g_smem_bytes = (unsigned)smem_bytes;
-        memset(smem, 0xA5, smem_bytes);  // shared memory is not zero-initialised
-        g_fibers.assign(nthr, Fiber{});
-        g_warps.assign((nthr + 31) / 32, Warp{});
-        g_ready.clear();
-        g_n_barrier = 0;
-        g_n_done = 0;
-        for (int t = 0; t < nthr; ++t) {
-            Fiber& f = g_fibers[t];
-            f.tid = t;
-            f.state = RUNNABLE;
-            void** top = reinterpret_cast<void**>(g_stacks[t] + kStackBytes);  // 16-byte aligned
-            void** sp = top - 8;
-            for (int i = 0; i < 8; ++i) sp[i] = nullptr;
-            sp[6] = reinterpret_cast<void*>(&fiber_main);  // "return address" of the first switch into the fiber
-            f.sp = sp;
-            g_ready.push_back(t);
+    g_block_idx = uint3{b, 0, 0};
+    g_smem = smem;
+    g_smem_bytes = (unsigned)smem_bytes;
+    memset(smem, 0xA5, smem_bytes);  // shared memory is not zero-initialised
+    g_fibers.assign(nthr, Fiber{});
+    g_warps.assign((nthr + 31) / 32, Warp{});
+    g_ready.clear();
+    g_n_barrier = 0;
+    g_n_done = 0;
+    for (int t = 0; t < nthr; ++t) {
+        Fiber& f = g_fibers[t];
+        f.tid = t;
+        f.state = RUNNABLE;
+        void** top = reinterpret_cast<void**>(g_stacks[t] + kStackBytes);  // 16-byte aligned
+        void** sp = top - 8;
+        for (int i = 0; i < 8; ++i) sp[i] = nullptr;
+        sp[6] = reinterpret_cast<void*>(&fiber_main);  // "return address" of the first switch into the fiber
+        f.sp = sp;
+        g_ready.push_back(t);
+    }
+    while (g_n_done < nthr) {
+        if (!g_ready.empty()) {  // resume a runnable fiber picked at random
+            const size_t i = rnd() % g_ready.size();
+            const int t = g_ready[i];
+            g_ready[i] = g_ready.back();
+            g_ready.pop_back();
+            g_cur = &g_fibers[t];
+            emu_switch(&g_sched_sp, g_cur->sp);
+            continue;
         }
-        while (g_n_done < nthr) {
-            if (!g_ready.empty()) {  // resume a runnable fiber picked at random
-                const size_t i = rnd() % g_ready.size();
-                const int t = g_ready[i];
-                g_ready[i] = g_ready.back();
-                g_ready.pop_back();
-                g_cur = &g_fibers[t];
-                emu_switch(&g_sched_sp, g_cur->sp);
-                continue;
-            }
-            if (g_n_barrier && g_n_barrier == nthr - g_n_done) {  // every live thread has arrived
-                for (Fiber& f : g_fibers) if (f.state == AT_BARRIER) { f.state = RUNNABLE; g_ready.push_back(f.tid); }
-                g_n_barrier = 0;
-                continue;
-            }
-            int nb = 0, nw = 0;
-            for (Fiber& f : g_fibers) { nb += f.state == AT_BARRIER; nw += f.state == AT_WARP; }
-            fprintf(stderr, "cuda_emu: DEADLOCK in block %u: %d threads at __syncthreads, %d in warp collectives, %d done of %d\n",
-                    b, nb, nw, g_n_done, nthr);
-            abort();
+        if (g_n_barrier && g_n_barrier == nthr - g_n_done) {  // every live thread has arrived
+            for (Fiber& f : g_fibers) if (f.state == AT_BARRIER) { f.state = RUNNABLE; g_ready.push_back(f.tid); }
+            g_n_barrier = 0;
+            continue;
         }
+        int nb = 0, nw = 0;
+        for (Fiber& f : g_fibers) { nb += f.state == AT_BARRIER; nw += f.state == AT_WARP; }
+        fprintf(stderr, "cuda_emu: DEADLOCK in block %u: %d threads at __syncthreads, %d in warp collectives, %d done of %d\n",
+                b, nb, nw, g_n_done, nthr);
+        abort();
     }
     g_cur = nullptr;
     g_smem = nullptr;
-    munmap(smem_base, smem_map);
+}
+
+void launch(dim3 grid, dim3 block, size_t smem_bytes, const std::function<void()>& body)
+{
+    const int nthr = (int)block.x;
+    g_block_dim = block;
+    g_grid_dim = grid;
+    g_body = &body;
+    const int workers = (int)std::min<unsigned>((unsigned)std::max(g_workers, 1), grid.x);
+    std::atomic<unsigned> next{0};
+    auto worker = [&](int wid) {
+        g_rng = g_seed ^ (0x9E3779B97F4A7C15ull * (unsigned long long)(wid + 1));
+        if (!g_rng) g_rng = 1;
+        size_t smem_map = 0; void* smem_base = nullptr;
+        unsigned char* smem = static_cast<unsigned char*>(guarded(smem_bytes ? smem_bytes : 16, &smem_map, &smem_base));
+        for (unsigned b = next.fetch_add(1); b < grid.x; b = next.fetch_add(1)) run_cta(b, nthr, smem, smem_bytes);
+        munmap(smem_base, smem_map);
+        if (workers > 1) {  // a worker thread ends with the launch: give its fiber stacks back
+            for (unsigned char* st : g_stacks) munmap(st, kStackBytes);
+            g_stacks.clear();
+        }
+    };
+    if (workers <= 1) {
+        worker(0);
+    } else {
+        std::vector<std::thread> th;
+        for (int w = 0; w < workers; ++w) th.emplace_back(worker, w);
+        for (auto& t : th) t.join();
+    }
 }
 
 }  // namespace cuda_emu
@@ -280,8 +311,9 @@ extern "C" const char* cuda_emu_first_violation(void) { return cuda_emu::g_first
 extern "C" void cuda_emu_reset_violations(void) { cuda_emu::g_violations = 0; cuda_emu::g_first_violation[0] = 0; }
 extern "C" void cuda_emu_configure(unsigned long long seed, int preempt_per_1024, unsigned smem_window)
 {
-    cuda_emu::g_rng = 0x9E3779B97F4A7C15ull ^ (seed * 0xD1342543DE82EF95ull);
-    if (!cuda_emu::g_rng) cuda_emu::g_rng = 1;
+    cuda_emu::g_seed = 0x9E3779B97F4A7C15ull ^ (seed * 0xD1342543DE82EF95ull);
     cuda_emu::g_preempt_per_1024 = preempt_per_1024;
     cuda_emu::g_smem_window = smem_window;
 }
+// CTAs of a grid that run at the same time, each on its own OS thread (1 = one after another)
+extern "C" void cuda_emu_set_workers(int n) { cuda_emu::g_workers = n < 1 ? 1 : n; }

@@ -42,14 +42,14 @@ static inline uint4 make_uint4(unsigned x, unsigned y, unsigned z, unsigned w) {
 #define __noinline__ __attribute__((noinline))
 #define __launch_bounds__(...)
 #define __align__(n) alignas(n)
-#define __shared__ static /* one CTA at a time: a function-local static is per-CTA state */
+#define __shared__ static thread_local /* one CTA at a time per OS thread: a function-local static is per-CTA state */
 
 namespace cuda_emu {
 
 struct Fiber;
-extern Fiber* g_cur;           // the fiber that is running
-extern unsigned char* g_smem;  // dynamic shared memory of the running CTA
-extern unsigned g_smem_bytes;
+extern thread_local Fiber* g_cur;           // the fiber that is running (per OS thread: one CTA at a time on each)
+extern thread_local unsigned char* g_smem;  // dynamic shared memory of the running CTA
+extern thread_local unsigned g_smem_bytes;
 extern unsigned g_smem_window; // shared-window address of g_smem[0] (what cvta.to.shared returns for it)
 extern dim3 g_block_dim, g_grid_dim;
 extern long long g_violations; // failed address checks (never performed)
@@ -93,13 +93,31 @@ template <typename T> static inline T __shfl_down_sync(unsigned mask, T v, unsig
 template <typename T> static inline T __shfl_xor_sync(unsigned mask, T v, int m) { return emu_shfl(cuda_emu::W_SHFL_XOR, mask, v, m); }
 static inline unsigned __match_any_sync(unsigned mask, unsigned v) { return (unsigned)cuda_emu::warp_collective(cuda_emu::W_MATCH_ANY, mask, v, 0); }
 
-// ------------------------------------------------------------------ atomics (one OS thread: plain read-modify-write)
-template <typename T, typename U> static inline T atomicAdd(T* p, U v) { cuda_emu::maybe_yield(); const T old = *p; *p = (T)(old + (T)v); return old; }
-template <typename T, typename U> static inline T atomicOr(T* p, U v) { cuda_emu::maybe_yield(); const T old = *p; *p = (T)(old | (T)v); return old; }
-template <typename T, typename U> static inline T atomicMax(T* p, U v) { cuda_emu::maybe_yield(); const T old = *p; if ((T)v > old) *p = (T)v; return old; }
-template <typename T, typename U> static inline T atomicMin(T* p, U v) { cuda_emu::maybe_yield(); const T old = *p; if ((T)v < old) *p = (T)v; return old; }
-template <typename T, typename U, typename V> static inline T atomicCAS(T* p, U cmp, V val) { cuda_emu::maybe_yield(); const T old = *p; if (old == (T)cmp) *p = (T)val; return old; }
-template <typename T, typename U> static inline T atomicExch(T* p, U v) { cuda_emu::maybe_yield(); const T old = *p; *p = (T)v; return old; }
+// ------------------------------------------------------------------ atomics (real ones: CTAs may run on several OS threads)
+template <typename T, typename U> static inline T atomicAdd(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_fetch_add(p, (T)v, __ATOMIC_SEQ_CST); }
+template <typename T, typename U> static inline T atomicOr(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_fetch_or(p, (T)v, __ATOMIC_SEQ_CST); }
+template <typename T, typename U, typename V> static inline T atomicCAS(T* p, U cmp, V val)
+{
+    cuda_emu::maybe_yield();
+    T expected = (T)cmp;
+    __atomic_compare_exchange_n(p, &expected, (T)val, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST);
+    return expected;  // the value that was there
+}
+template <typename T, typename U> static inline T atomicMax(T* p, U v)
+{
+    cuda_emu::maybe_yield();
+    T old = __atomic_load_n(p, __ATOMIC_SEQ_CST);
+    while ((T)v > old && !__atomic_compare_exchange_n(p, &old, (T)v, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST)) {}
+    return old;
+}
+template <typename T, typename U> static inline T atomicMin(T* p, U v)
+{
+    cuda_emu::maybe_yield();
+    T old = __atomic_load_n(p, __ATOMIC_SEQ_CST);
+    while ((T)v < old && !__atomic_compare_exchange_n(p, &old, (T)v, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST)) {}
+    return old;
+}
+template <typename T, typename U> static inline T atomicExch(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_exchange_n(p, (T)v, __ATOMIC_SEQ_CST); }
 
 // ------------------------------------------------------------------ memory and arithmetic intrinsics
 template <typename T> static inline T __ldg(const T* p) { return *p; }

@@ -67,10 +67,12 @@ def lib():
     return _lib
 
 
-def configure(seed: int = 0, preempt_per_1024: int = 0, smem_window: int = 1024):
+def configure(seed: int = 0, preempt_per_1024: int = 0, smem_window: int = 1024, workers: int = 1):
     """Schedule seed, chance of a switch at every atomic / cache-bypassing access, shared-window address of the dynamic
-    shared memory (what cvta.to.shared returns for its first byte)."""
+    shared memory (what cvta.to.shared returns for its first byte), CTAs of a grid that run at the same time (each on its
+    own OS thread; 1 = one after another)."""
     lib().cuda_emu_configure(seed, preempt_per_1024, smem_window)
+    lib().cuda_emu_set_workers(workers)
 
 
 def theta_window(p):

@@ -106,6 +106,23 @@ def test_shared_window_offset(window):
     assert g["deferred"] == (0 if window < 4096 and window % 256 == 0 else 2)
 
 
+@pytest.mark.parametrize("workers,flags", [(4, 0), (6, E.FLAG_SMALL_LISTS), (5, E.FLAG_GENERAL_ONLY)])
+def test_concurrent_ctas(workers, flags):
+    """Several persistent CTAs at the same time, each on its own OS thread: they share the work counter, the deferred list and
+    the status word through real atomics, and each uses its own slab of the general kernel's global scratch (blockIdx > 0)."""
+    E.configure(seed=7, workers=workers)
+    try:
+        wl, u, v, offsets, kinds = mixed_batch(3, 48, seed=29)
+        p = params_of(wl)
+        g = E.run(p, u, v, offsets, E.HOUGH_U16, flags=flags, want_acc=False)
+        o = oracle_run(p, u, v, offsets, want_acc=False)
+        assert_same(g, o, p)
+        if flags == 0:
+            assert g["deferred"] == kinds.count("count>1023")
+    finally:
+        E.configure(seed=1, workers=1)
+
+
 def test_many_events_per_cta():
     """The model runs the CTAs of a grid one after another, so the first CTA of the persistent grid processes EVERY event:
     per-event resets (halos, lists, histogram, control block), tile reuse across events, the work counter."""
