@@ -285,6 +285,7 @@ def run_ours(args, cfg=None, hits_idx=None, grid_idx=None, quiet=False):
     barrier()
     launches = H.hough_plan_launch_count(plan) - launches0
     clocks = sampler.stop()
+    deferred = int(H.hough_plan_debug_counters(plan)[15])          # events the fast kernel handed to the general kernel (last step)
     ms_total = max_over_ranks(e_begin.elapsed_time(e_end))
     ms_step = ms_total / args.steps
     ms_find = statistics.mean(e[0].elapsed_time(e[1]) for e in evs)
@@ -336,8 +337,9 @@ def run_ours(args, cfg=None, hits_idx=None, grid_idx=None, quiet=False):
         sm_max = (clocks.get("sm_max_mhz") or 1965.0) * 1e6
         # diagnostic second ceiling: a vote needs at least 5 issued instructions (2 IMAD, SHF, LOP3, RED) on 4 schedulers / SM
         alu_peak = info["n_sm"] * 4 * sm_max / 5.0 * 32
-        roofline = {"bound": "smem_atomic", "kernel": "hough_fast_kernel (hough_find_clusters)" if info["fast_groups"] else
-                    "hough_event_kernel (hough_find_clusters)",
+        roofline = {"bound": "smem_atomic",
+                    "kernel": ("hough_fast_kernel (hough_find_clusters)" if info["fast_groups"] and 2 * deferred <= n_events else
+                               "hough_event_kernel (hough_find_clusters; %d of %d events)" % (deferred if info["fast_groups"] else n_events, n_events)),
                     "achieved": achieved / 1e9, "peak": peak_ops / 1e9, "unit": "Gatomic/s", "frac": achieved / peak_ops,
                     "peak_source": "hough_measure_smem_atomic_peak, measured live on this GPU (nothing but conflict-free "
                                    "red.shared.add.u32, %.0f MHz); MEASURED_PEAKS.json has no shared-memory figure" % peak_mhz,
@@ -377,7 +379,7 @@ def run_ours(args, cfg=None, hits_idx=None, grid_idx=None, quiet=False):
                                                      "(shard.shard_events), no collective on the data path; per-event results "
                                                      "all-gathered afterwards" if strong else
                                                      f"events sharded over {world} GPU(s), no collective"),
-                                     "plan": info, "status_word": status, "gen_s": round(t_gen, 1)}),
+                                     "plan": info, "status_word": status, "deferred_events": deferred, "gen_s": round(t_gen, 1)}),
                 "kernel_ms": {"hough_find_clusters": ms_find, "hough_assign_hits": ms_assign},
                 "ms_per_step_median": statistics.median(step_ms), "ms_per_step_best": min(step_ms),     # this rank's steps
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
