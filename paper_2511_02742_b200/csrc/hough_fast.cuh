@@ -258,6 +258,11 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
     // boundary (the host sized the fixed-point range for that).  If the driver ever places it elsewhere, nothing is
     // computed here: every event this CTA fetches goes to the general kernel.
     const bool fold_ok = tile_base < 4096u && (tile_base & ((1u << k) - 1u)) == 0u;
+    // Dense workloads (every bin on: e.g. 2000 hits on a 128 x 128 grid) overflow the lists event after event; the vote spent on
+    // such an event is wasted, the general kernel redoes it.  After kGiveUpRun capacity overflows in a row this CTA hands the next
+    // kGiveUpSkip events over untouched, then tries again.  Block-uniform registers; changes which kernel computes an event, never a result.
+    constexpr int kGiveUpRun = 8, kGiveUpSkip = 64;
+    int overflow_run = 0, skip_left = 0;
 
     while (true) {
         __syncthreads();  // previous event fully done
@@ -271,6 +276,11 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
 
         const long long g0 = offsets[e], g1 = offsets[e + 1];
         const long long ne64 = g1 - g0;
+        if (skip_left > 0 && ne64 > 0) {
+            --skip_left;
+            if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
+            continue;
+        }
         if (!fold_ok || g0 < 0 || ne64 < 0 || ne64 > (long long)P.fHB || ne64 > (long long)P.max_hits_per_event) {
             // bad offsets, or more hits than the staging buffer: the general kernel handles (and flags) it
             if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
@@ -564,8 +574,10 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
         const int n_on = sh.n_on, n_pk = sh.n_peaks;
         if (give_up || n_pk > P.fPCAP) {
             if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
+            if (++overflow_run >= kGiveUpRun) { overflow_run = 0; skip_left = kGiveUpSkip; }
             continue;
         }
+        overflow_run = 0;
         // the tile is dead: its first ONCAP words become the root tags
         for (int i = tid; i < n_on; i += nthr) if (HB(P, i, P.f_tile_bytes >> 2, 150)) roottag[i] = 0;
 

@@ -465,3 +465,15 @@ def test_restricted_theta_window():
             k = min(int(o["n_found"][e]), p.max_candidates)
             assert g["cands"][e, :k].tobytes() == o["cands"][e, :k].tobytes()
     assert (o["cands"]["theta"][0, :8] >= math.pi / 4 - 1e-6).all() and (o["cands"]["theta"][0, :8] < 3 * math.pi / 4).all()
+
+
+def test_dense_workload_is_handed_over_after_a_run_of_overflows():
+    """2000 hits on a 128 x 128 grid switch (nearly) every bin on: each event overflows the fast kernel's lists.  After eight
+    overflows in a row a CTA hands the next 64 events over without voting on them; results are the general kernel's either way."""
+    wl = synth.workload(4, 2, 0)
+    b = synth.generate(wl, 0, 30)
+    p = params_of(wl)
+    g = E.run(p, b.u, b.v, b.offsets, want_acc=False)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert g["info"]["fast_groups"] > 0 and g["deferred"] == 30
