@@ -477,3 +477,27 @@ def test_dense_workload_is_handed_over_after_a_run_of_overflows():
     o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
     assert_same(g, o, p)
     assert g["info"]["fast_groups"] > 0 and g["deferred"] == 30
+
+
+def tiny_events(n_events, seed):
+    """Many tiny events on a 64 x 64 grid: one short track (12 collinear hits) plus a few noise hits each."""
+    rng = np.random.default_rng(seed)
+    n = 16
+    m, c = rng.uniform(-1, 1, n_events), rng.uniform(-100, 100, n_events)
+    uu = np.tile(np.linspace(-90, 90, 12), (n_events, 1))
+    vv = m[:, None] * uu + c[:, None]
+    u = np.concatenate([uu, rng.uniform(-94, 94, (n_events, n - 12))], axis=1).astype(np.float32).ravel()
+    v = np.concatenate([vv, rng.uniform(-194, 194, (n_events, n - 12))], axis=1).astype(np.float32).ravel()
+    return u, v, np.arange(0, n * n_events + 1, n, dtype=np.int64)
+
+
+def test_general_kernel_epoch_tags_wrap():
+    """The general kernel tags its union-find words with a 10-bit per-CTA epoch instead of clearing its global scratch per event;
+    after 1023 events of one CTA the tags would repeat, so the slab is cleared and the epoch restarts.  The model's first CTA
+    takes every event: 1100 events cross that point."""
+    p = std_params(64, 64, T=8, K=8)
+    u, v, offsets = tiny_events(1100, seed=61)
+    g = E.run(p, u, v, offsets, flags=E.FLAG_GENERAL_ONLY, want_acc=False)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert (o["n_found"] >= 1).mean() > 0.9

@@ -417,3 +417,21 @@ def test_restricted_theta_window():
         for e in range(200):
             k = min(int(o["n_found"][e]), p.max_candidates)
             assert g["cands"][e, :k].tobytes() == o["cands"][e, :k].tobytes()
+
+
+def test_general_kernel_epoch_tags_wrap():
+    """More than 1023 events per persistent CTA through the general kernel: its 10-bit epoch tags wrap, the per-CTA union-find
+    slab is cleared and the epoch restarts.  320,000 tiny events: more than 1023 per CTA on average even with 296 CTAs."""
+    from test_emulated_kernels import tiny_events
+    p = std_params(64, 64, T=8, K=8)
+    n = 320000
+    u, v, offsets = tiny_events(n, seed=62)
+    g = gpu_run(p, u, v, offsets, want_vote=False, flags=H.HOUGH_FLAG_GENERAL_ONLY)
+    assert g["info"]["n_ctas"] * 1023 < n and g["bounds_violations"] == 0 and g["status"] == 0
+    assert_path(g, fast=False, deferred=0)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    np.testing.assert_array_equal(g["n_found"], o["n_found"])
+    np.testing.assert_array_equal(g["labels"], o["labels"])
+    kept = np.arange(p.max_candidates)[None, :] < np.minimum(o["n_found"], p.max_candidates)[:, None]
+    for f in INT_FIELDS + ("theta", "rho"):
+        np.testing.assert_array_equal(g["cands"][f][kept], o["cands"][f][kept], err_msg=f)
