@@ -92,15 +92,38 @@ def _llround(x: float) -> int:
     return n if x >= 0 else -n
 
 
+def _tables(p: Params, F: int):
+    """(M, C_q, S_q, O_q, W_q) for a given F."""
+    H = p.hit_frac_bits
+    d_rho = (p.rho_max - p.rho_min) / p.n_rho
+    M = float(2 ** (F - H)) / d_rho if F >= H else 1.0 / (float(2 ** (H - F)) * d_rho)
+    Cq = tuple(_llround(math.cos(p.theta_of(t)) * M) for t in range(p.n_theta))
+    Sq = tuple(_llround(math.sin(p.theta_of(t)) * M) for t in range(p.n_theta))
+    Oq = _llround(-p.rho_min * float(2 ** F) / d_rho)
+    Wq = _llround(p.assign_window * float(2 ** F) / d_rho)
+    return M, Cq, Sq, Oq, Wq
+
+
+def int32_proof(p: Params, F: int) -> bool:
+    """Every intermediate of O3 and O7 fits int32 for EVERY valid hit: q_max (max_t |C_q| + |S_q|) + |O_q| <= 2^31 - 1 with
+    q_max = floor(coord_max 2^H + 1/2) >= |u_q|, |v_q| (the corner hits attain it), and (n_rho + 1) 2^F <= 2^31 - 1."""
+    _, Cq, Sq, Oq, _ = _tables(p, F)
+    qmax = math.floor(p.coord_max * float(2 ** p.hit_frac_bits) + 0.5)
+    max_cs = max(abs(c) + abs(s) for c, s in zip(Cq, Sq))
+    return qmax * max_cs + abs(Oq) <= INT32_MAX and (p.n_rho + 1) * 2 ** F <= INT32_MAX
+
+
 def default_frac_bits(p: Params) -> int:
-    """O2: largest F <= 24 with span * 2^F <= 2^31 - 1,
-    span = max(sqrt(2) coord_max / d_rho + max(|rho_min|, |rho_max|) / d_rho + 2, n_rho + 1): every intermediate of O3 AND the
-    bin centres r 2^F + 2^(F-1) of O7 (r < n_rho) stay inside int32."""
+    """O2: the largest F <= 24 that keeps every intermediate inside int32.  Start from the closed form
+    span * 2^F <= 2^31 - 1, span = max(sqrt(2) coord_max / d_rho + max(|rho_min|, |rho_max|) / d_rho + 2, n_rho + 1)
+    (which already is the answer unless d_rho is far below the hit resolution 2^-H), then lower F until int32_proof holds."""
     d_rho = (p.rho_max - p.rho_min) / p.n_rho
     span = math.sqrt(2.0) * p.coord_max / d_rho + max(abs(p.rho_min), abs(p.rho_max)) / d_rho + 2.0
     span = max(span, float(p.n_rho + 1))
     F = 24
     while F > 0 and span * float(2 ** F) > float(INT32_MAX):
+        F -= 1
+    while F > 1 and not int32_proof(p, F):
         F -= 1
     return F
 
@@ -111,11 +134,7 @@ def constants(p: Params) -> Constants:
     H = p.hit_frac_bits
     F = p.acc_frac_bits if p.acc_frac_bits >= 0 else default_frac_bits(p)
     d_rho = (p.rho_max - p.rho_min) / p.n_rho
-    M = float(2 ** (F - H)) / d_rho if F >= H else 1.0 / (float(2 ** (H - F)) * d_rho)
-    Cq = tuple(_llround(math.cos(p.theta_of(t)) * M) for t in range(p.n_theta))
-    Sq = tuple(_llround(math.sin(p.theta_of(t)) * M) for t in range(p.n_theta))
-    Oq = _llround(-p.rho_min * float(2 ** F) / d_rho)
-    Wq = _llround(p.assign_window * float(2 ** F) / d_rho)
+    M, Cq, Sq, Oq, Wq = _tables(p, F)
     return Constants(H, F, d_rho, M, Cq, Sq, Oq, Wq)
 
 

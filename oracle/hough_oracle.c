@@ -61,6 +61,24 @@ static double ho_theta(const ho_params_t* p, int t)
 
 static double pow2i(int e) { return ldexp(1.0, e); }
 
+/* Every intermediate of O3 and O7 fits int32 for every valid hit: q_max (max_t |C_q| + |S_q|) + |O_q| <= 2^31 - 1 with
+ * q_max = floor(coord_max 2^H + 1/2), and (n_rho + 1) 2^F <= 2^31 - 1. */
+static int ho_int32_proof(const ho_params_t* p, int F)
+{
+    const int H = p->hit_frac_bits;
+    const double d_rho = (p->rho_max - p->rho_min) / p->n_rho;
+    const double M = pow2i(F - H) / d_rho;
+    double max_cs = 0.0;
+    for (int t = 0; t < p->n_theta; ++t) {
+        const double th = ho_theta(p, t);
+        const double cs = fabs((double)llround(cos(th) * M)) + fabs((double)llround(sin(th) * M));
+        if (cs > max_cs) max_cs = cs;
+    }
+    const double qmax = floor(p->coord_max * pow2i(H) + 0.5);
+    const double oq = fabs((double)llround(-p->rho_min * pow2i(F) / d_rho));
+    return qmax * max_cs + oq <= 2147483647.0 && ((double)p->n_rho + 1.0) * pow2i(F) <= 2147483647.0;
+}
+
 int ho_default_frac_bits(const ho_params_t* p)
 {
     double d_rho = (p->rho_max - p->rho_min) / p->n_rho;
@@ -69,6 +87,7 @@ int ho_default_frac_bits(const ho_params_t* p)
     int F = 24;
     if (span < (double)p->n_rho + 1.0) span = (double)p->n_rho + 1.0;  /* bin centres r 2^F + 2^(F-1), r < n_rho (O7) */
     while (F > 0 && span * pow2i(F) > 2147483647.0) --F;
+    while (F > 1 && !ho_int32_proof(p, F)) --F;  /* d_rho far below the hit resolution: the closed form is not enough */
     return F;
 }
 

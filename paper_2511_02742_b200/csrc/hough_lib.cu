@@ -233,15 +233,31 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
 
     // ---- fixed-point constants (host double precision, llround = half away from zero)
     const double d_rho = (d->rho_max - d->rho_min) / d->n_rho;
+    // int32 proof of a given F: |u_q C| + |v_q S| + |O_q| <= 2^31 - 1 for every valid hit (|u_q|, |v_q| <= q_max = floor(coord_max 2^H
+    // + 1/2); the corner hits attain q_max (|C| + |S|)), and the bin centres r 2^F + 2^(F-1) of the assignment fit too
+    auto int32_proof = [&](int f) {
+        const double m = ldexp(1.0, f - H) / d_rho;
+        double max_cs = 0.0;
+        for (int t = 0; t < d->n_theta; ++t) {
+            const double th = th_lo + (th_hi - th_lo) * t / d->n_theta;
+            const double cs = fabs((double)llround(cos(th) * m)) + fabs((double)llround(sin(th) * m));
+            if (cs > max_cs) max_cs = cs;
+        }
+        const double qmax = floor(d->coord_max * ldexp(1.0, H) + 0.5);
+        const double oq = fabs((double)llround(-d->rho_min * ldexp(1.0, f) / d_rho));
+        return qmax * max_cs + oq <= 2147483647.0 && ((double)d->n_rho + 1.0) * ldexp(1.0, f) <= 2147483647.0;
+    };
     int F = d->acc_frac_bits;
-    if (F < 0) {
+    if (F < 0) {  // the largest F <= 24 that passes the proof: closed form first (O2), then down until it holds
         const double amin = fabs(d->rho_min), amax = fabs(d->rho_max);
         double span = sqrt(2.0) * d->coord_max / d_rho + (amin > amax ? amin : amax) / d_rho + 2.0;
-        if (span < (double)d->n_rho + 1.0) span = (double)d->n_rho + 1.0;  // the bin centres r 2^F + 2^(F-1) of the assignment fit too
+        if (span < (double)d->n_rho + 1.0) span = (double)d->n_rho + 1.0;
         F = 24;
         while (F > 0 && span * ldexp(1.0, F) > 2147483647.0) --F;
+        while (F > 1 && !int32_proof(F)) --F;
     }
     if (F > 30 || F < 1) return HOUGH_ERANGE;
+    if (fabs(d->rho_min) * ldexp(1.0, F) / d_rho > 2147483646.0 || !int32_proof(F)) return HOUGH_ERANGE;
     const double M = ldexp(1.0, F - H) / d_rho;
     const double oq_d = -d->rho_min * ldexp(1.0, F) / d_rho;
     const double wq_d = d->assign_window * ldexp(1.0, F) / d_rho;
@@ -255,21 +271,13 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     p->desc.acc_frac_bits = F;
     p->h_cos.resize(d->n_theta);
     p->h_sin.resize(d->n_theta);
-    long long max_cs = 0;
     for (int t = 0; t < d->n_theta; ++t) {
         const double th = th_lo + (th_hi - th_lo) * t / d->n_theta;  // [0, pi): pi t / n_theta bit for bit
         const long long c = llround(cos(th) * M), s = llround(sin(th) * M);
         p->h_cos[t] = (int32_t)c;
         p->h_sin[t] = (int32_t)s;
-        const long long cs = llabs(c) + llabs(s);
-        if (cs > max_cs) max_cs = cs;
     }
-    // int32 proof: |u_q C| + |v_q S| + |O_q| <= 2^31 - 1 for every valid hit, and bin centres r 2^F + 2^(F-1) fit too
-    const long long qmax = (long long)floor(d->coord_max * ldexp(1.0, H)) + 1;
-    if ((double)qmax * (double)max_cs + fabs((double)Oq) > 2147483647.0 || ((double)d->n_rho + 1.0) * ldexp(1.0, F) > 2147483647.0) {
-        delete p;
-        return HOUGH_ERANGE;
-    }
+    const long long qmax = (long long)floor(d->coord_max * ldexp(1.0, H) + 0.5);
 
     // ---- launch configuration
     int dev_count = 0;

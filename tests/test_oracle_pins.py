@@ -178,6 +178,20 @@ def test_p1c_theta_window(impl):
     assert acc[int(tb)].max() == 48 and abs(float(thf) - (math.pi / 4 + (math.pi / 2) * int(tb) / 256)) < 1e-6
 
 
+def test_p1b_default_frac_bits_passes_the_int32_proof_on_exotic_plans():
+    """d_rho far below the hit resolution 2^-H (found by tests/emu/fuzz_parity.py): the closed-form span is not enough there, F is
+    lowered until q_max (|C_q| + |S_q|) + |O_q| fits for the corner hits; the corner hits then really do stay inside int32."""
+    for p in (D.Params(180, 1000, -3.6, 2.4, 1.0, 1, 0.006, 16, 0, -1), D.Params(32, 568, -1.0, 1.0, 1.0, 5, 0.001, 16, 0, -1),
+              D.Params(64, 700, -0.4, 0.4, 50.0, 2, 0.01, 8, 3, -1), D.Params(90, 300, -2.0, 3.0, 256.0, 2, 0.1, 8, 0, -1)):
+        F = D.default_frac_bits(p)
+        assert D.int32_proof(p, F) and (F == 24 or not D.int32_proof(p, F + 1) or
+                                        (math.sqrt(2.0) * p.coord_max + max(abs(p.rho_min), abs(p.rho_max))) / ((p.rho_max - p.rho_min) / p.n_rho) * 2 ** (F + 1) > 2 ** 31 - 1)
+        assert C.constants(p)[1] == F
+        c = np.float32(p.coord_max)
+        acc = D.vote_event(np.array([c, -c, c, -c], np.float32), np.array([c, c, -c, -c], np.float32), p)      # asserts the bound inside
+        np.testing.assert_array_equal(acc, C.vote_event(np.array([c, -c, c, -c], np.float32), np.array([c, c, -c, -c], np.float32), p))
+
+
 # ----------------------------------------------------------------------------- P2 table CRC
 def test_p2_table_crc32(impl):
     for n_theta, crc in read_golden_table("table_crc32.txt"):
