@@ -435,3 +435,66 @@ def test_general_kernel_epoch_tags_wrap():
     kept = np.arange(p.max_candidates)[None, :] < np.minimum(o["n_found"], p.max_candidates)[:, None]
     for f in INT_FIELDS + ("theta", "rho"):
         np.testing.assert_array_equal(g["cands"][f][kept], o["cands"][f][kept], err_msg=f)
+
+
+# ----------------------------------------------------------------------------- BASELINE sizes, bench.py's launch configuration
+def _gen_chunk(job):
+    from paper_2511_02742_b200 import synth as S
+    b = S.generate_chunk(job[0], job[1])
+    return b.u, b.v, b.offsets
+
+
+def generate_all(wl, n_events):
+    """The first n_events events of a workload, chunks generated in worker processes (spawned: CUDA is alive in this one)."""
+    import multiprocessing as mp
+    import os
+    n_chunks = (n_events + synth.CHUNK_EVENTS - 1) // synth.CHUNK_EVENTS
+    jobs = [(wl, c) for c in range(n_chunks)]
+    if n_chunks > 2:
+        with mp.get_context("spawn").Pool(min(n_chunks, max(1, (os.cpu_count() or 2) - 1))) as pool:
+            parts = pool.map(_gen_chunk, jobs, chunksize=1)
+    else:
+        parts = [_gen_chunk(j) for j in jobs]
+    u, v = np.concatenate([p[0] for p in parts]), np.concatenate([p[1] for p in parts])
+    offs, base = [np.zeros(1, np.int64)], 0
+    for p in parts:
+        offs.append(p[2][1:] + base); base += int(p[2][-1])
+    offsets = np.concatenate(offs)[: n_events + 1]
+    return np.ascontiguousarray(u[: offsets[-1]]), np.ascontiguousarray(v[: offsets[-1]]), np.ascontiguousarray(offsets)
+
+
+@pytest.mark.parametrize("cfg,hits_idx,grid_idx,n_sample", [(1, 0, 0, 0), (2, 0, 0, 0), (3, 0, 0, 1500), (4, 1, 2, 1500), (4, 2, 0, 300), (4, 0, 3, 1500)])
+def test_full_size_in_the_bench_launch_configuration(cfg, hits_idx, grid_idx, n_sample):
+    """Every event of the config at BASELINE.json's size in ONE launch, exactly as bench.py times it (100,000 events of cfg3 on
+    the persistent grid: some 675 events per CTA).  Configs 1 and 2 are compared event by event; for cfg3 and the config-4 cells
+    the oracle computes a random sample of events one by one (n_found, records, labels), plus two properties that hold at any
+    size: every label is -1 or a kept slot, and no event was handed over that the workload's statistics say should not be."""
+    wl = synth.workload(cfg, hits_idx, grid_idx)
+    u, v, offsets = generate_all(wl, wl.n_events)
+    E = wl.n_events
+    p = params_of(wl)
+    dt = H.HOUGH_U16 if wl.count_dtype == "u16" else H.HOUGH_I32
+    g = gpu_run(p, u, v, offsets, dt, want_vote=False)
+    assert g["bounds_violations"] == 0 and g["status"] == 0
+    if (cfg, hits_idx) != (4, 2):                      # (2000 hits on 128 x 128 switch every bin on: the general kernel's case)
+        assert_path(g, fast=True, deferred=0)
+    kept = np.minimum(g["n_found"], p.max_candidates)
+    lab_event = np.repeat(np.arange(E), np.diff(offsets))
+    assert (g["labels"] >= -1).all() and (g["labels"] < kept[lab_event]).all()
+    rng = np.random.default_rng(99)
+    events = np.arange(E) if n_sample == 0 else np.sort(rng.choice(E, n_sample, replace=False))
+    if n_sample == 0:
+        o = oracle_run(p, u, v, offsets, want_acc=False)
+        np.testing.assert_array_equal(g["n_found"], o["n_found"])
+        np.testing.assert_array_equal(g["labels"], o["labels"])
+        mask = np.arange(p.max_candidates)[None, :] < np.minimum(o["n_found"], p.max_candidates)[:, None]
+        for f in INT_FIELDS + ("theta", "rho"):
+            np.testing.assert_array_equal(g["cands"][f][mask], o["cands"][f][mask], err_msg=f)
+        return
+    for e in events:
+        a, z = int(offsets[e]), int(offsets[e + 1])
+        o = C.run_batch(u[a:z], v[a:z], np.array([0, z - a], np.int64), p)
+        k = min(int(o["n_found"][0]), p.max_candidates)
+        assert int(g["n_found"][e]) == int(o["n_found"][0]), e
+        assert g["cands"][e, :k].tobytes() == o["cands"][0, :k].tobytes(), e
+        np.testing.assert_array_equal(g["labels"][a:z], o["labels"], err_msg=str(e))
