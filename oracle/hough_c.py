@@ -28,7 +28,8 @@ class _CParams(ctypes.Structure):
                 ("rho_min", ctypes.c_double), ("rho_max", ctypes.c_double), ("coord_max", ctypes.c_double),
                 ("vote_threshold", ctypes.c_int32), ("assign_window", ctypes.c_double),
                 ("max_candidates", ctypes.c_int32), ("hit_frac_bits", ctypes.c_int32), ("acc_frac_bits", ctypes.c_int32),
-                ("theta_min", ctypes.c_double), ("theta_max", ctypes.c_double)]
+                ("theta_min", ctypes.c_double), ("theta_max", ctypes.c_double),
+                ("theta_wrap", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 def build(force: bool = False) -> str:
@@ -70,7 +71,7 @@ def lib():
 
 def _cp(p: Params) -> _CParams:
     return _CParams(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.vote_threshold, p.assign_window,
-                    p.max_candidates, p.hit_frac_bits, p.acc_frac_bits, p.theta_min, p.theta_max)
+                    p.max_candidates, p.hit_frac_bits, p.acc_frac_bits, p.theta_min, p.theta_max, int(p.theta_wrap), 0)
 
 
 def _ptr(a: Optional[np.ndarray]):

@@ -55,6 +55,7 @@ class Params:
     acc_frac_bits: int = -1       # F; < 0 -> default formula
     theta_min: float = 0.0        # theta window [theta_min, theta_max) in radians; the paper's is [0, pi)
     theta_max: float = math.pi
+    theta_wrap: bool = False      # O4 / O5 treat theta = pi as theta = 0 with rho mirrored (reading B9); default: no wrap
 
     def theta_of(self, t: int) -> float:
         """theta_t = theta_min + (theta_max - theta_min) t / n_theta (left bin edge); for the default window pi t / n_theta."""
@@ -181,29 +182,52 @@ def _key(acc: np.ndarray, t: int, r: int, n_rho: int) -> Tuple[int, int]:
 _NEIGH8 = ((-1, -1), (-1, 0), (-1, 1), (0, -1), (0, 1), (1, -1), (1, 0), (1, 1))
 
 
+def check_theta_wrap(p: Params) -> None:
+    """Reading B9: the line (theta + pi, rho) IS the line (theta, -rho) (Eq. 4.1: cos and sin change sign together).  With the
+    paper's window [0, pi) and a rho range symmetric about 0, bin (t, r) continued past the last theta row is therefore bin
+    (t - n_theta, n_rho - 1 - r).  Wrap needs exactly that window and range, and n_theta >= 3 so that the row before and the
+    row after a row are different rows."""
+    assert p.theta_min == 0.0 and p.theta_max == math.pi and p.rho_min == -p.rho_max and p.n_theta >= 3, \
+        "theta_wrap needs theta in [0, pi), rho_min = -rho_max and n_theta >= 3"
+
+
+def neighbours8(t: int, r: int, p: Params) -> List[Tuple[int, int]]:
+    """The in-grid 8-neighbours of bin (t, r).  Without wrap: the rectangle's.  With wrap (B9) the theta rows form a ring with
+    a twist: the step from row n_theta - 1 to row 0 (and back) mirrors the rho bin, r -> n_rho - 1 - r."""
+    out = []
+    for dt, dr in _NEIGH8:
+        tt, rr = t + dt, r + dr
+        if p.theta_wrap and tt < 0:
+            tt, rr = tt + p.n_theta, p.n_rho - 1 - rr
+        elif p.theta_wrap and tt >= p.n_theta:
+            tt, rr = tt - p.n_theta, p.n_rho - 1 - rr
+        if 0 <= tt < p.n_theta and 0 <= rr < p.n_rho:
+            out.append((tt, rr))
+    return out
+
+
 def peaks(acc: np.ndarray, p: Params) -> List[Tuple[int, int]]:
-    """O4: on(b) <=> acc(b) >= T;  peak(b) <=> on(b) and key(b) > key(n) for all in-grid 8-neighbours (no wrap)."""
+    """O4: on(b) <=> acc(b) >= T;  peak(b) <=> on(b) and key(b) > key(n) for all in-grid 8-neighbours (no wrap unless
+    p.theta_wrap, reading B9: then the neighbours across the theta seam count too)."""
+    if p.theta_wrap:
+        check_theta_wrap(p)
     out = []
     for t in range(p.n_theta):
         for r in range(p.n_rho):
             if acc[t, r] < p.vote_threshold:
                 continue
             kb = _key(acc, t, r, p.n_rho)
-            is_peak = True
-            for dt, dr in _NEIGH8:
-                tt, rr = t + dt, r + dr
-                if 0 <= tt < p.n_theta and 0 <= rr < p.n_rho and _key(acc, tt, rr, p.n_rho) > kb:
-                    is_peak = False
-                    break
-            if is_peak:
+            if all(_key(acc, tt, rr, p.n_rho) < kb for tt, rr in neighbours8(t, r, p)):
                 out.append((t, r))
     return out
 
 
 def components(acc: np.ndarray, p: Params) -> Tuple[np.ndarray, List[Tuple[Tuple[int, int], int]]]:
-    """O5: 8-connected components of the on-mask (no wrap), by union-find.
+    """O5: 8-connected components of the on-mask (no wrap unless p.theta_wrap, reading B9), by union-find.
     Returns (label array: component id per bin or -1, list per component of (root bin = max-key bin, n_bins))."""
     nt, nr = p.n_theta, p.n_rho
+    if p.theta_wrap:
+        check_theta_wrap(p)
     parent = {}
 
     def find(x):
@@ -219,9 +243,8 @@ def components(acc: np.ndarray, p: Params) -> Tuple[np.ndarray, List[Tuple[Tuple
                 continue
             b = t * nr + r
             parent[b] = b
-            for dt, dr in ((-1, -1), (-1, 0), (-1, 1), (0, -1)):       # already-visited half of the 8-neighbourhood
-                tt, rr = t + dt, r + dr
-                if 0 <= tt < nt and 0 <= rr < nr and on[tt, rr]:
+            for tt, rr in neighbours8(t, r, p):
+                if tt * nr + rr < b and on[tt, rr]:                    # the neighbours already visited (smaller linear index)
                     ra, rb = find(tt * nr + rr), find(b)
                     if ra != rb:
                         parent[max(ra, rb)] = min(ra, rb)

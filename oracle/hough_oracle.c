@@ -36,6 +36,8 @@ typedef struct {
     int32_t hit_frac_bits;
     int32_t acc_frac_bits; /* < 0: default */
     double theta_min, theta_max; /* theta window in radians; (0, 0) = the paper's [0, pi) */
+    int32_t theta_wrap;          /* != 0: O4 / O5 continue past the last theta row into row 0 with rho mirrored (reading B9) */
+    int32_t reserved;
 } ho_params_t;
 
 typedef struct { /* 32 bytes, the record layout the public ABI documents */
@@ -164,6 +166,18 @@ static int key_greater(const int32_t* acc, int64_t b, int64_t n)
     return b < n;
 }
 
+/* Linear index of the 8-neighbour (t + dt, r + dr) of bin (t, r), or -1 if it is outside the grid.  With theta_wrap (reading
+ * B9: the line (theta + pi, rho) is the line (theta, -rho), so for theta in [0, pi) and rho_min = -rho_max the row after the last
+ * one is row 0 with the rho bins in reverse order) the step across the seam mirrors the rho bin: r -> n_rho - 1 - r. */
+static int64_t ho_neighbour(const ho_params_t* p, int t, int r, int dt, int dr)
+{
+    int tt = t + dt, rr = r + dr;
+    if (p->theta_wrap && tt < 0) { tt += p->n_theta; rr = p->n_rho - 1 - rr; }
+    else if (p->theta_wrap && tt >= p->n_theta) { tt -= p->n_theta; rr = p->n_rho - 1 - rr; }
+    if (tt < 0 || tt >= p->n_theta || rr < 0 || rr >= p->n_rho) return -1;
+    return (int64_t)tt * p->n_rho + rr;
+}
+
 typedef struct { int64_t L; int32_t votes; } ho_peak_t;
 
 static int peak_cmp(const void* x, const void* y)
@@ -178,7 +192,11 @@ int ho_find_clusters_event(const ho_params_t* p, const int32_t* acc, ho_cand_t* 
 {
     const int nt = p->n_theta, nr = p->n_rho, T = p->vote_threshold, K = p->max_candidates;
     const int64_t nb = (int64_t)nt * nr;
-    /* O5: flood fill of the on-mask, 8-connectivity, no wrap */
+    if (p->theta_wrap) { /* B9 needs the paper's window, a symmetric rho range and three distinct rows around every row */
+        const int default_window = (p->theta_min == 0.0 && (p->theta_max == 0.0 || p->theta_max == HO_PI));
+        if (!default_window || p->rho_min != -p->rho_max || nt < 3) return HO_EARG;
+    }
+    /* O5: flood fill of the on-mask, 8-connectivity (no wrap unless theta_wrap) */
     int32_t* comp = (int32_t*)malloc(sizeof(int32_t) * nb);     /* component id per bin, -1 = off/unvisited */
     int64_t* stack = (int64_t*)malloc(sizeof(int64_t) * nb);
     int64_t* comp_root = (int64_t*)malloc(sizeof(int64_t) * (nb / 1 + 1));
@@ -201,9 +219,8 @@ int ho_find_clusters_event(const ho_params_t* p, const int32_t* acc, ho_cand_t* 
             for (int dt = -1; dt <= 1; ++dt)
                 for (int dr = -1; dr <= 1; ++dr) {
                     if (!dt && !dr) continue;
-                    int tt = t + dt, rr = r + dr;
-                    if (tt < 0 || tt >= nt || rr < 0 || rr >= nr) continue;
-                    int64_t n = (int64_t)tt * nr + rr;
+                    int64_t n = ho_neighbour(p, t, r, dt, dr);
+                    if (n < 0) continue;
                     if (acc[n] >= T && comp[n] < 0) { comp[n] = n_comp; stack[sp++] = n; }
                 }
         }
@@ -219,9 +236,9 @@ int ho_find_clusters_event(const ho_params_t* p, const int32_t* acc, ho_cand_t* 
         for (int dt = -1; dt <= 1 && is_peak; ++dt)
             for (int dr = -1; dr <= 1; ++dr) {
                 if (!dt && !dr) continue;
-                int tt = t + dt, rr = r + dr;
-                if (tt < 0 || tt >= nt || rr < 0 || rr >= nr) continue;
-                if (key_greater(acc, (int64_t)tt * nr + rr, b)) { is_peak = 0; break; }
+                int64_t n = ho_neighbour(p, t, r, dt, dr);
+                if (n < 0 || n == b) continue;
+                if (key_greater(acc, n, b)) { is_peak = 0; break; }
             }
         if (is_peak) { pk[np_].L = b; pk[np_].votes = acc[b]; ++np_; }
     }

@@ -397,6 +397,155 @@ def test_p9_peaks_are_the_strict_local_maxima_brute_force(impl):
     assert got == exp and nf == len(exp)
 
 
+# ----------------------------------------------------------------------------- P9w theta wrap (reading B9)
+def _stack_of_copies(acc, k):
+    """The accumulator continued over theta in [-k pi, (k + 1) pi): copy j is the grid itself for even j and the grid with its
+    rho bins reversed for odd j (the line (theta + pi, rho) is the line (theta, -rho)).  -> (stack, row of copy 0's row 0)"""
+    copies = [acc if j % 2 == 0 else acc[:, ::-1] for j in range(-k, k + 1)]
+    return np.concatenate(copies, axis=0), k * acc.shape[0]
+
+
+def _wrap_params(n_theta, n_rho, T, K=None):
+    return D.Params(n_theta, n_rho, -1.0, 1.0, 1.0, T, 0.1, K or n_theta * n_rho, theta_wrap=True)
+
+
+@pytest.mark.parametrize("shape,density,seed", [((5, 6), 0.5, 1), ((7, 9), 0.35, 2), ((3, 8), 0.6, 3), ((12, 10), 0.2, 4),
+                                                 ((6, 7), 0.95, 5), ((9, 4), 0.05, 6)])
+def test_p9w_wrap_equals_plain_rules_on_the_unrolled_theta_axis(impl, shape, density, seed):
+    """Brute force: unroll the theta axis (stack mirrored copies), apply the NO-wrap definitions there with library labelling,
+    and read the result off copy 0.  A simple path visits each bin at most once and moves at most one row per step, so
+    n_rho + 1 copies on either side hold a lift of every path that starts in copy 0."""
+    from scipy import ndimage
+
+    rng = np.random.default_rng(seed)
+    n_theta, n_rho, T = shape[0], shape[1], 3
+    acc = _random_acc(rng, n_theta, n_rho, T, density)
+    p = _wrap_params(n_theta, n_rho, T)
+    cands, nf = impl.clusters(acc, p)
+    tup = cands_as_tuples(cands)
+    k = n_rho + 1
+    stack, row0 = _stack_of_copies(acc, k)
+    lin = np.arange(n_theta * n_rho).reshape(n_theta, n_rho)                 # linear index of the bin a stack cell is a copy of
+    lin_stack, _ = _stack_of_copies(lin, k)
+    # peaks: strict local maxima of copy 0 inside the stack under (count, -linear index of the original bin)
+    exp_peaks = set()
+    for t in range(n_theta):
+        for r in range(n_rho):
+            if acc[t, r] < T:
+                continue
+            me = (int(acc[t, r]), -int(lin[t, r]))
+            ok = True
+            for dt, dr in itertools.product((-1, 0, 1), repeat=2):
+                tt, rr = row0 + t + dt, r + dr
+                if (dt, dr) != (0, 0) and 0 <= rr < n_rho and (int(stack[tt, rr]), -int(lin_stack[tt, rr])) > me:
+                    ok = False
+            if ok:
+                exp_peaks.add((t, r))
+    assert {(t, r) for t, r, *_ in tup} == exp_peaks and nf == len(exp_peaks)
+    # components: two bins belong together iff copy 0 of one is connected to SOME copy of the other
+    lab, _ = ndimage.label(stack >= T, structure=np.ones((3, 3), int))
+    classes = {}                                                             # stack label -> set of original bins
+    for (tt, rr), l in np.ndenumerate(lab):
+        if l:
+            classes.setdefault(l, set()).add(int(lin_stack[tt, rr]))
+    for s, (t, r, votes, root, nb) in enumerate(tup):
+        members = classes[lab[row0 + t, r]]
+        assert nb == len(members), (s, t, r)
+        rt, rr = tup[root][0], tup[root][1]
+        assert rt * n_rho + rr in members
+        assert (tup[root][2], -(rt * n_rho + rr)) == max((int(acc.flat[b]), -b) for b in members)
+
+
+def test_p9w_hand_built_seam_cases(impl):
+    """Special cases small enough to check by eye: two on bins, one in the first and one in the last theta row."""
+    n_theta, n_rho, T = 6, 10, 5
+    plain, wrap = D.Params(n_theta, n_rho, -1.0, 1.0, 1.0, T, 0.1, 8), _wrap_params(n_theta, n_rho, T, 8)
+
+    def both(cells):
+        acc = np.zeros((n_theta, n_rho), np.int32)
+        for (t, r), c in cells.items():
+            acc[t, r] = c
+        return cands_as_tuples(impl.clusters(acc, plain)[0]), cands_as_tuples(impl.clusters(acc, wrap)[0])
+
+    r = 3
+    m = n_rho - 1 - r                                                        # the bin that (0, r) continues into past the seam
+    for dm in (-1, 0, 1):                                                    # straight and diagonal neighbours across the seam
+        pl, wr = both({(0, r): 10, (n_theta - 1, m + dm): 9})
+        assert pl == [(0, r, 10, 0, 1), (n_theta - 1, m + dm, 9, 1, 1)]
+        assert wr == [(0, r, 10, 0, 2)]
+        pl, wr = both({(0, r): 9, (n_theta - 1, m + dm): 10})
+        assert wr == [(n_theta - 1, m + dm, 10, 0, 2)]
+        pl, wr = both({(0, r): 10, (n_theta - 1, m + dm): 10})               # a tie: the smaller linear index wins
+        assert wr == [(0, r, 10, 0, 2)]
+    for dm in (-2, 2):                                                       # two bins apart: not neighbours
+        pl, wr = both({(0, r): 10, (n_theta - 1, m + dm): 9})
+        assert wr == pl == [(0, r, 10, 0, 1), (n_theta - 1, m + dm, 9, 1, 1)]
+    pl, wr = both({(0, r): 10, (n_theta - 1, r): 9})                         # same rho bin, NOT mirrored: r = 3 continues into 6, not 3
+    assert wr == pl and len(wr) == 2
+    pl, wr = both({(0, 0): 10, (n_theta - 1, n_rho - 1): 9, (0, n_rho - 1): 8, (n_theta - 1, 0): 7})   # the corners pair up crosswise
+    assert wr == [(0, 0, 10, 0, 2), (0, n_rho - 1, 8, 1, 2)]
+
+
+def test_p9w_a_vertical_track_is_one_cluster_with_wrap_and_two_without(impl):
+    """Textbook case: hits on the line u = c (theta = 0) vote (0, bin(c)) n times, and the rows just below theta = pi see the
+    same line at rho = -c: the ridge of a single track crosses the seam.  Without wrap it is two clusters, each with its own
+    best candidate; with wrap (B9) one cluster whose size is the sum, rooted at the better of the two."""
+    n_theta, n_rho = 90, 64
+    c = -256.0 + 45.5 * (512.0 / n_rho)                                      # centre of rho bin 45
+    v = np.linspace(-30, 30, 25).astype(np.float32)
+    u = np.full_like(v, c)
+    base = dict(n_theta=n_theta, n_rho=n_rho, rho_min=-256.0, rho_max=256.0, coord_max=256.0, vote_threshold=12,
+                assign_window=8.0, max_candidates=16)
+    acc = impl.vote(u, v, D.Params(**base))
+    assert acc[0, 45] == len(u) and acc[n_theta - 1, n_rho - 1 - 45] >= 12   # both sides of the seam are on
+    plain = cands_as_tuples(impl.clusters(acc, D.Params(**base))[0])
+    wrapped = cands_as_tuples(impl.clusters(acc, D.Params(**base, theta_wrap=True))[0])
+    assert {(t, r) for t, r, *_ in wrapped} <= {(t, r) for t, r, *_ in plain}    # more neighbours can only remove peaks
+    roots_plain = sorted({rt for *_, rt, _ in plain})
+    assert len(roots_plain) == 2 and plain[0][:2] == (0, 45)
+    near, far = (plain[rt] for rt in roots_plain)
+    assert near[0] < 10 and far[0] > n_theta - 10                            # one cluster on either side of the seam
+    assert {rt for *_, rt, _ in wrapped} == {0} and wrapped[0][:3] == (0, 45, len(u))
+    assert all(nb == near[4] + far[4] for *_, nb in wrapped)
+
+
+def test_p9w_rotating_the_theta_origin_changes_nothing(impl):
+    """Invariant: with wrap the theta axis has no preferred origin.  Rotating the rows by s (rows pushed past the seam come
+    back mirrored) maps peaks to peaks and clusters to clusters when no two bins tie (all counts distinct)."""
+    rng = np.random.default_rng(9)
+    n_theta, n_rho, T = 8, 11, 40
+    acc = rng.permutation(n_theta * n_rho).reshape(n_theta, n_rho).astype(np.int32)
+    p = _wrap_params(n_theta, n_rho, T)
+    ref = cands_as_tuples(impl.clusters(acc, p)[0])
+    for s in (1, 3, 7):
+        rot = np.concatenate([acc[s:], acc[:s, ::-1]], axis=0)
+        back = lambda t, r: (t + s, r) if t + s < n_theta else (t + s - n_theta, n_rho - 1 - r)
+        got = cands_as_tuples(impl.clusters(rot, p)[0])
+        assert sorted((back(t, r), vt, nb) for t, r, vt, _, nb in got) == sorted(((t, r), vt, nb) for t, r, vt, _, nb in ref)
+        assert sorted(back(*got[rt][:2]) for *_, rt, _ in got) == sorted(ref[rt][:2] for *_, rt, _ in ref)
+
+
+def test_p9w_wrap_needs_the_paper_window_and_a_symmetric_rho_range():
+    acc = np.zeros((6, 6), np.int32)
+    for bad in (D.Params(6, 6, -1.0, 2.0, 1.0, 1, 0.1, 4, theta_wrap=True), D.Params(2, 6, -1.0, 1.0, 1.0, 1, 0.1, 4, theta_wrap=True),
+                D.Params(6, 6, -1.0, 1.0, 1.0, 1, 0.1, 4, theta_min=0.0, theta_max=1.0, theta_wrap=True)):
+        with pytest.raises(AssertionError):
+            D.find_clusters_event(acc, bad)
+        with pytest.raises(RuntimeError):
+            C.find_clusters_event(acc, bad)
+
+
+def test_p9w_both_oracles_agree_with_wrap_on_generated_events():
+    for seed in (1, 2, 3):
+        u, v = small_event(seed, n_tracks=3, n_noise=30)
+        u[:10] = np.float32(-93.5)                                           # a vertical track: its ridge crosses the seam
+        p = std_params(64, 64, T=8, K=32, theta_wrap=True)
+        a1, c1, n1, l1 = run(DefImpl, u, v, p)
+        a2, c2, n2, l2 = run(CImpl, u, v, p)
+        assert (a1 == a2).all() and n1 == n2 and cands_as_tuples(c1) == cands_as_tuples(c2) and (l1 == l2).all()
+        assert [float(c.theta) for c in c1] == [float(c["theta"]) for c in c2]
+
+
 # ----------------------------------------------------------------------------- P10 brute force over hit pairs
 def _collinear_event(rng, p, groups, n_per_group, n_free):
     """Exactly collinear groups on bin-centre lines (well separated), plus general-position hits."""
