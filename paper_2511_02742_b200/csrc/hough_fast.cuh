@@ -374,7 +374,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
                             m = (((gx >> 15) | (gx >> 30)) & 3u) | ((((gy >> 15) | (gy >> 30)) & 3u) << 2) |
                                 ((((gz >> 15) | (gz >> 30)) & 3u) << 4) | ((((gw >> 15) | (gw >> 30)) & 3u) << 6);
                             // a count above 1023 does not fit the packed entries: the general kernel takes the event
-                            if (((w.x + oadd) | (w.y + oadd) | (w.z + oadd) | (w.w + oadd)) & 0x80008000u) sh.defer = 1;
+                            if (((w.x + oadd) | (w.y + oadd) | (w.z + oadd) | (w.w + oadd)) & 0x80008000u) atomicOr(&sh.defer, 1);  // several threads may: no plain store
                         }
                         // theta rows beyond n_theta hold no votes (checked_vote masks them), so m needs no masking
                         if (halo_lane && HB(P, hp - halo_cur, P.n_rho, 120)) {  // the row's two last counts are the next strip's count halo

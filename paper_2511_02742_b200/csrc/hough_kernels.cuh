@@ -111,7 +111,12 @@ __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)
 __device__ __forceinline__ void red_add_shared(uint32_t addr, uint32_t v)
 {
 #ifdef HOUGH_EMU
-    if (uint32_t* w = static_cast<uint32_t*>(emu_shared_ptr(addr, 4, "red.shared.add.u32 outside the CTA's shared memory"))) *w += v;
+    uint32_t* w = static_cast<uint32_t*>(emu_shared_ptr(addr, 4, "red.shared.add.u32 outside the CTA's shared memory"));
+#ifdef HOUGH_EMU_TSAN  // race-detector build of the host model: the detector must see an atomic
+    if (w) __atomic_fetch_add(w, v, __ATOMIC_RELAXED);
+#else
+    if (w) *w += v;  // fibers of a CTA share one OS thread and switch only at barriers and collectives
+#endif
 #else
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 #endif

@@ -2,7 +2,12 @@
 the host CUDA model of cuda_emu.h.  TEST INFRASTRUCTURE -- NOT PART OF THE PRODUCT (nothing under paper_2511_02742_b200/
 imports or loads it).
 
-    python tests/emu/build_emu.py [--force]
+    python tests/emu/build_emu.py [--force] [--tsan]
+
+--tsan builds tests/emu/libhough_emu_tsan.so, the race-detector variant: the kernel sources are compiled with
+-fsanitize=thread and -DHOUGH_EMU_TSAN (every CUDA thread a ThreadSanitizer fiber, see cuda_emu.cpp); the model itself
+(cuda_emu.cpp) is NOT instrumented, so the detector sees the kernels' memory accesses and only the synchronisation CUDA
+defines.  Load it in a process started with LD_PRELOAD=$(gcc -print-file-name=libtsan.so); tests/emu/race_check.py does.
 """
 from __future__ import annotations
 
@@ -14,8 +19,29 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(os.path.dirname(_HERE))
 _CSRC = os.path.join(_ROOT, "paper_2511_02742_b200", "csrc")
 LIB = os.path.join(_HERE, "libhough_emu.so")
+LIB_TSAN = os.path.join(_HERE, "libhough_emu_tsan.so")
 DEPENDS = [os.path.join(_HERE, "cuda_emu.h"), os.path.join(_HERE, "cuda_emu.cpp"), os.path.join(_ROOT, "include", "hough.h")] + \
           [os.path.join(_CSRC, f) for f in sorted(os.listdir(_CSRC))]
+
+
+def build_tsan(force: bool = False, csrc: str = _CSRC, out: str = LIB_TSAN) -> str:
+    """csrc / out: race_check.py --self-test builds a copy of the sources with one barrier taken out."""
+    if not force and csrc == _CSRC and os.path.exists(out) and all(os.path.getmtime(d) <= os.path.getmtime(out) for d in DEPENDS):
+        return out
+    tmp = out + f".tmp{os.getpid()}"
+    common = ["g++", "-std=c++17", "-O1", "-g", "-fPIC", "-ffp-contract=off", "-fno-strict-aliasing", "-DHOUGH_EMU", "-DHOUGH_EMU_TSAN",
+              "-DHOUGH_BOUNDS", "-Wno-unknown-pragmas", "-I", _HERE]
+    obj_model, obj_kernels = tmp + ".model.o", tmp + ".kernels.o"
+    try:
+        subprocess.check_call(common + ["-c", os.path.join(_HERE, "cuda_emu.cpp"), "-o", obj_model])
+        subprocess.check_call(common + ["-fsanitize=thread", "-c", "-x", "c++", os.path.join(csrc, "hough_lib.cu"), "-o", obj_kernels])
+        subprocess.check_call(["g++", "-shared", "-fsanitize=thread", obj_kernels, obj_model, "-o", tmp, "-pthread"])
+    finally:
+        for o in (obj_model, obj_kernels):
+            if os.path.exists(o):
+                os.remove(o)
+    os.replace(tmp, out)
+    return out
 
 
 def build(force: bool = False) -> str:
@@ -32,4 +58,4 @@ def build(force: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv))
+    print((build_tsan if "--tsan" in sys.argv else build)(force="--force" in sys.argv))

@@ -37,6 +37,26 @@ emu_switch:
 .size emu_switch,.-emu_switch
 )");
 
+// Race-detector build (-DHOUGH_EMU_TSAN, g++ -fsanitize=thread; tests/emu/build_emu.py --tsan): every CUDA thread is a
+// ThreadSanitizer fiber of its own, switched WITHOUT synchronisation, so that two CUDA threads of a CTA are concurrent for the
+// detector exactly where CUDA says they are: the only happens-before edges inside a CTA are __syncthreads (all threads),
+// __syncwarp (the lanes of the mask) and program order.  ballot / shuffle / match exchange registers and order no memory.
+// Atomics are relaxed (cuda_emu.h), as CUDA's are.  Kernel launches and the CTAs that follow one another on one worker are
+// ordered through the scheduler (they reuse the same host memory as "shared memory").
+#ifdef HOUGH_EMU_TSAN
+extern "C" {
+void* __tsan_get_current_fiber(void);
+void* __tsan_create_fiber(unsigned flags);
+void __tsan_destroy_fiber(void* fiber);
+void __tsan_switch_to_fiber(void* fiber, unsigned flags);  // flags 1: no synchronisation on the switch
+void __tsan_acquire(void* addr);
+void __tsan_release(void* addr);
+}
+#define TSAN_ONLY(...) __VA_ARGS__
+#else
+#define TSAN_ONLY(...)
+#endif
+
 namespace cuda_emu {
 
 enum State { RUNNABLE, AT_BARRIER, AT_WARP, DONE };
@@ -56,6 +76,7 @@ struct Pending {  // one warp collective in flight
 
 struct Warp {
     Pending pend[8];
+    char sync_token[8];  // race-detector build: what the lanes of a __syncwarp release and acquire, one per slot of pend
     unsigned long long res[32];
     unsigned gen[32];  // per lane: bumped when the collective the lane waits in completes
 };
@@ -85,6 +106,11 @@ static int g_preempt_per_1024 = 0;  // chance (in 1/1024) that an atomic / cache
 static int g_workers = 1;
 static char g_first_violation[256] = "";
 static std::mutex g_mutex;
+#ifdef HOUGH_EMU_TSAN
+static thread_local std::vector<void*> g_tsan_fibers;  // one detector context per CUDA thread slot of this worker
+static thread_local void* g_tsan_sched = nullptr;
+static thread_local char g_barrier_token, g_start_token, g_done_token;  // addresses only: what release / acquire name
+#endif
 
 static unsigned rnd()
 {
@@ -106,7 +132,11 @@ void violation(const char* what, unsigned long long a, unsigned long long lim)
     ++g_violations;
 }
 
-static void yield_to_scheduler() { emu_switch(&g_cur->sp, g_sched_sp); }
+static void yield_to_scheduler()
+{
+    TSAN_ONLY(__tsan_switch_to_fiber(g_tsan_sched, 1);)
+    emu_switch(&g_cur->sp, g_sched_sp);
+}
 
 void maybe_yield()
 {
@@ -120,7 +150,9 @@ void sync_threads()
 {
     g_cur->state = AT_BARRIER;
     ++g_n_barrier;
+    TSAN_ONLY(__tsan_release(&g_barrier_token);)  // every thread releases before the first one leaves ...
     yield_to_scheduler();
+    TSAN_ONLY(__tsan_acquire(&g_barrier_token);)  // ... and acquires all of them
 }
 
 static void complete(Warp& w, Pending& p)
@@ -169,6 +201,7 @@ unsigned long long warp_collective(WarpOp op, unsigned mask, unsigned long long 
     p->val[lane] = val;
     p->arg[lane] = arg;
     p->arrived |= 1u << lane;
+    TSAN_ONLY(char* const token = &w.sync_token[p - w.pend]; if (op == W_SYNC) __tsan_release(token);)
     if (p->arrived == p->mask) {
         const unsigned m = p->mask;
         complete(w, *p);
@@ -179,12 +212,15 @@ unsigned long long warp_collective(WarpOp op, unsigned mask, unsigned long long 
         f->state = AT_WARP;
         while (w.gen[lane] == my_gen) yield_to_scheduler();
     }
+    TSAN_ONLY(if (op == W_SYNC) __tsan_acquire(token);)
     return w.res[lane];
 }
 
 static void fiber_main()
 {
+    TSAN_ONLY(__tsan_acquire(&g_start_token);)  // after the scheduler's set-up of this CTA (and whatever ran before it)
     (*g_body)();
+    TSAN_ONLY(__tsan_release(&g_done_token);)
     g_cur->state = DONE;
     ++g_n_done;
     for (;;) yield_to_scheduler();
@@ -234,6 +270,11 @@ static void run_cta(unsigned b, int nthr, unsigned char* smem, size_t smem_bytes
     g_smem = smem;
     g_smem_bytes = (unsigned)smem_bytes;
     memset(smem, 0xA5, smem_bytes);  // shared memory is not zero-initialised
+#ifdef HOUGH_EMU_TSAN
+    if (!g_tsan_sched) g_tsan_sched = __tsan_get_current_fiber();
+    while ((int)g_tsan_fibers.size() < nthr) g_tsan_fibers.push_back(__tsan_create_fiber(0));
+    __tsan_release(&g_start_token);
+#endif
     g_fibers.assign(nthr, Fiber{});
     g_warps.assign((nthr + 31) / 32, Warp{});
     g_ready.clear();
@@ -257,6 +298,7 @@ static void run_cta(unsigned b, int nthr, unsigned char* smem, size_t smem_bytes
             g_ready[i] = g_ready.back();
             g_ready.pop_back();
             g_cur = &g_fibers[t];
+            TSAN_ONLY(__tsan_switch_to_fiber(g_tsan_fibers[t], 1);)
             emu_switch(&g_sched_sp, g_cur->sp);
             continue;
         }
@@ -271,6 +313,7 @@ static void run_cta(unsigned b, int nthr, unsigned char* smem, size_t smem_bytes
                 b, nb, nw, g_n_done, nthr);
         abort();
     }
+    TSAN_ONLY(__tsan_acquire(&g_done_token);)  // the CTA's accesses happen before whatever this worker does next
     g_cur = nullptr;
     g_smem = nullptr;
 }
@@ -293,6 +336,11 @@ void launch(dim3 grid, dim3 block, size_t smem_bytes, const std::function<void()
         if (workers > 1) {  // a worker thread ends with the launch: give its fiber stacks back
             for (unsigned char* st : g_stacks) munmap(st, kStackBytes);
             g_stacks.clear();
+#ifdef HOUGH_EMU_TSAN
+            for (void* f : g_tsan_fibers) __tsan_destroy_fiber(f);
+            g_tsan_fibers.clear();
+            g_tsan_sched = nullptr;
+#endif
         }
     };
     if (workers <= 1) {

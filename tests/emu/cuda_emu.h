@@ -38,7 +38,13 @@ static inline uint4 make_uint4(unsigned x, unsigned y, unsigned z, unsigned w) {
 #define __global__
 #define __device__
 #define __host__
+#ifdef HOUGH_EMU_TSAN  // race-detector build: device functions keep their frames, so that a suppression can name one
+#define __forceinline__ inline __attribute__((noinline))
+#define EMU_ATOMIC_ORDER __ATOMIC_RELAXED  // CUDA's atomics order nothing; a stronger order here would hide races from the detector
+#else
 #define __forceinline__ inline __attribute__((always_inline))
+#define EMU_ATOMIC_ORDER __ATOMIC_SEQ_CST
+#endif
 #define __noinline__ __attribute__((noinline))
 #define __launch_bounds__(...)
 #define __align__(n) alignas(n)
@@ -94,30 +100,30 @@ template <typename T> static inline T __shfl_xor_sync(unsigned mask, T v, int m)
 static inline unsigned __match_any_sync(unsigned mask, unsigned v) { return (unsigned)cuda_emu::warp_collective(cuda_emu::W_MATCH_ANY, mask, v, 0); }
 
 // ------------------------------------------------------------------ atomics (real ones: CTAs may run on several OS threads)
-template <typename T, typename U> static inline T atomicAdd(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_fetch_add(p, (T)v, __ATOMIC_SEQ_CST); }
-template <typename T, typename U> static inline T atomicOr(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_fetch_or(p, (T)v, __ATOMIC_SEQ_CST); }
+template <typename T, typename U> static inline T atomicAdd(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_fetch_add(p, (T)v, EMU_ATOMIC_ORDER); }
+template <typename T, typename U> static inline T atomicOr(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_fetch_or(p, (T)v, EMU_ATOMIC_ORDER); }
 template <typename T, typename U, typename V> static inline T atomicCAS(T* p, U cmp, V val)
 {
     cuda_emu::maybe_yield();
     T expected = (T)cmp;
-    __atomic_compare_exchange_n(p, &expected, (T)val, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST);
+    __atomic_compare_exchange_n(p, &expected, (T)val, false, EMU_ATOMIC_ORDER, EMU_ATOMIC_ORDER);
     return expected;  // the value that was there
 }
 template <typename T, typename U> static inline T atomicMax(T* p, U v)
 {
     cuda_emu::maybe_yield();
-    T old = __atomic_load_n(p, __ATOMIC_SEQ_CST);
-    while ((T)v > old && !__atomic_compare_exchange_n(p, &old, (T)v, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST)) {}
+    T old = __atomic_load_n(p, EMU_ATOMIC_ORDER);
+    while ((T)v > old && !__atomic_compare_exchange_n(p, &old, (T)v, false, EMU_ATOMIC_ORDER, EMU_ATOMIC_ORDER)) {}
     return old;
 }
 template <typename T, typename U> static inline T atomicMin(T* p, U v)
 {
     cuda_emu::maybe_yield();
-    T old = __atomic_load_n(p, __ATOMIC_SEQ_CST);
-    while ((T)v < old && !__atomic_compare_exchange_n(p, &old, (T)v, false, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST)) {}
+    T old = __atomic_load_n(p, EMU_ATOMIC_ORDER);
+    while ((T)v < old && !__atomic_compare_exchange_n(p, &old, (T)v, false, EMU_ATOMIC_ORDER, EMU_ATOMIC_ORDER)) {}
     return old;
 }
-template <typename T, typename U> static inline T atomicExch(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_exchange_n(p, (T)v, __ATOMIC_SEQ_CST); }
+template <typename T, typename U> static inline T atomicExch(T* p, U v) { cuda_emu::maybe_yield(); return __atomic_exchange_n(p, (T)v, EMU_ATOMIC_ORDER); }
 
 // ------------------------------------------------------------------ memory and arithmetic intrinsics
 template <typename T> static inline T __ldg(const T* p) { return *p; }

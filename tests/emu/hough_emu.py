@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CAND_DTYPE = np.dtype([("theta_bin", "<i4"), ("rho_bin", "<i4"), ("votes", "<i4"), ("cluster_root", "<i4"),
                        ("cluster_nbins", "<i4"), ("theta", "<f4"), ("rho", "<f4"), ("reserved", "<i4")])
 HOUGH_I32, HOUGH_U16 = 0, 1
-FLAG_GENERAL_ONLY, FLAG_SMALL_LISTS = 1, 2
+FLAG_GENERAL_ONLY, FLAG_SMALL_LISTS, FLAG_THETA_WRAP = 1, 2, 4
 
 
 class Desc(ctypes.Structure):
@@ -47,7 +47,10 @@ def lib():
         spec = importlib.util.spec_from_file_location("build_emu", os.path.join(_HERE, "build_emu.py"))
         mod = importlib.util.module_from_spec(spec)
         spec.loader.exec_module(mod)
-        L = ctypes.CDLL(mod.build())
+        # HOUGH_EMU_LIB=tsan: the race-detector build (the process must have been started with libtsan preloaded: race_check.py);
+        # HOUGH_EMU_LIB=/path/to.so: a library race_check.py --self-test built
+        which = os.environ.get("HOUGH_EMU_LIB", "")
+        L = ctypes.CDLL(mod.build_tsan() if which == "tsan" else (which if which else mod.build()))
         vp, i32 = ctypes.c_void_p, ctypes.c_int32
         L.hough_plan_create.argtypes = [ctypes.POINTER(Desc), ctypes.POINTER(vp)]
         L.hough_plan_destroy.argtypes = [vp]
@@ -105,6 +108,8 @@ def run(p, u, v, offsets, count_dtype=HOUGH_I32, want_acc=True, max_hpe=None, fl
     L.cuda_emu_reset_violations()
     E = len(offsets) - 1
     hpe = int(np.diff(offsets).max()) if E > 0 and len(u) else 0
+    if getattr(p, "theta_wrap", False):
+        flags |= FLAG_THETA_WRAP
     d = Desc(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.hit_frac_bits, p.acc_frac_bits, p.vote_threshold,
              p.assign_window, p.max_candidates, count_dtype, max(1, E), max(0, len(u)), max(hpe, 1) if max_hpe is None else max_hpe,
              flags, 0, *theta_window(p))
