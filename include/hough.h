@@ -54,7 +54,15 @@ enum { HOUGH_STATUS_EVENT_TOO_LONG = 1, HOUGH_STATUS_BAD_OFFSETS = 2,      /* bi
  *   HOUGH_FLAG_GENERAL_ONLY  every event goes through the general kernel (the shared-memory-only fast kernel is not used)
  *   HOUGH_FLAG_SMALL_LISTS   the fast kernel's per-event lists get their smallest capacities, so that ordinary events
  *                            overflow them and are handed to the general kernel (exercises that hand-over in tests) */
-enum { HOUGH_FLAG_GENERAL_ONLY = 1, HOUGH_FLAG_SMALL_LISTS = 2 };
+enum { HOUGH_FLAG_GENERAL_ONLY = 1, HOUGH_FLAG_SMALL_LISTS = 2,
+/*   HOUGH_FLAG_THETA_WRAP    DOES change results (a variant; reading B9): the line (theta + pi, rho)
+ *                            is the line (theta, -rho) (Eq. 4.1), so the theta rows close into a ring with a twist -- past the
+ *                            last row comes row 0 with its rho bins in reverse order.  With this flag local maxima (S2) and clusters
+ *                            (S3) see those neighbours too: bin (n_theta - 1, r) touches bins (0, n_rho - 1 - r + {-1, 0, 1}).  A
+ *                            track near theta = 0 is then one cluster instead of one at either end of the theta axis.  Needs the
+ *                            default theta window, rho_min = -rho_max and n_theta >= 3 (else HOUGH_EINVAL); every event goes through
+ *                            the general kernel; hough_find_tracks_peeloff and hough_find_two_stage do not accept such a plan. */
+       HOUGH_FLAG_THETA_WRAP = 4 };
 
 typedef struct hough_plan hough_plan_t;           /* opaque; created and destroyed by the library */
 

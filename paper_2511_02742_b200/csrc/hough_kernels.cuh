@@ -74,6 +74,8 @@ struct DevParams {
     uint32_t* csize;    // [n_ctas][n_bins]  component sizes, valid at union-find roots
     uint2* onlist;      // [n_ctas][n_bins]  (L, count) of every on bin
     uint2* peaks_ovf;   // [n_ctas][n_bins / 4 + 1] peaks beyond PCAP
+    uint32_t* first_rows;  // [n_ctas][2][n_rho]  counts of theta rows 0 and 1 of the event (theta_wrap only)
+    int theta_wrap;     // O4 / O5 continue past the last theta row into row 0 with rho mirrored (HOUGH_FLAG_THETA_WRAP, reading B9)
     uint32_t* epoch;    // [n_ctas]
     int* status;
     unsigned int* work_counter;
@@ -271,16 +273,32 @@ __device__ __forceinline__ uint32_t count_at(const DevParams& P, const unsigned 
     return halo[(tl + 2) * P.n_rho + r];
 }
 
+// Count of rho bin r of a theta row kept in global memory, seen from the other side of the theta seam (reading B9): the
+// row is read mirrored, r -> n_rho - 1 - r.
+__device__ __forceinline__ uint32_t mirrored_at(const DevParams& P, const uint32_t* row, int r)
+{
+    const int m = P.n_rho - 1 - r;
+    return (unsigned)m < (unsigned)P.n_rho ? __ldcg(row + m) : 0u;
+}
+
 // Strict local maximum under the total order key = (count, -L): neighbours with a smaller linear index
-// (previous theta row, or same row and r - 1) win ties.
+// (previous theta row, or same row and r - 1) win ties.  seam_row0 (theta_wrap, last theta row only): the counts of theta
+// row 0, which follows the last row mirrored and, having the smaller linear indices, wins ties.
 template <int CW>
-__device__ __forceinline__ bool is_peak(const DevParams& P, const unsigned char* tile, const uint32_t* halo, int tl, int r, uint32_t c)
+__device__ __forceinline__ bool is_peak(const DevParams& P, const unsigned char* tile, const uint32_t* halo, int tl, int r, uint32_t c,
+                                        const uint32_t* seam_row0 = nullptr)
 {
     if (count_at<CW>(P, tile, halo, tl - 1, r - 1) >= c) return false;
     if (count_at<CW>(P, tile, halo, tl - 1, r) >= c) return false;
     if (count_at<CW>(P, tile, halo, tl - 1, r + 1) >= c) return false;
     if (count_at<CW>(P, tile, halo, tl, r - 1) >= c) return false;
     if (count_at<CW>(P, tile, halo, tl, r + 1) > c) return false;
+    if (seam_row0) {
+        if (mirrored_at(P, seam_row0, r - 1) >= c) return false;
+        if (mirrored_at(P, seam_row0, r) >= c) return false;
+        if (mirrored_at(P, seam_row0, r + 1) >= c) return false;
+        return true;
+    }
     if (count_at<CW>(P, tile, halo, tl + 1, r - 1) > c) return false;
     if (count_at<CW>(P, tile, halo, tl + 1, r) > c) return false;
     if (count_at<CW>(P, tile, halo, tl + 1, r + 1) > c) return false;
@@ -328,6 +346,8 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
     uint32_t* csize = P.csize + (size_t)blockIdx.x * P.n_bins;
     uint2* onlist = P.onlist + (size_t)blockIdx.x * P.n_bins;
     uint2* peaks_ovf = P.peaks_ovf + (size_t)blockIdx.x * (P.n_bins / 4 + 1);
+    uint32_t* first_rows = P.first_rows + (size_t)blockIdx.x * 2 * P.n_rho;
+    const bool wrap = !DUMP && P.theta_wrap;
     uint32_t epoch = DUMP ? 0 : P.epoch[blockIdx.x];
 #ifdef HOUGH_PHASE_TIMERS
     long long pt_acc[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -436,6 +456,13 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
             }
 
             // ---------------- S2: threshold + local maxima
+            if (wrap && strip == 0) {  // theta rows 0 and 1 are needed again when the last theta row is known (reading B9)
+                for (int r = tid; r < P.n_rho; r += nthr) {
+                    __stcg(first_rows + r, tile_get<CW>(tile, P.S, r, 0));
+                    __stcg(first_rows + P.n_rho + r, tile_get<CW>(tile, P.S, r, 1));
+                }
+                __syncthreads();  // the last theta row may be in this very strip
+            }
             if (strip > 0) {  // deferred row: the last theta row of the previous strip, now that row 0 is known
                 for (int r = tid; r < P.n_rho; r += nthr) {
                     const uint32_t c = halo[P.n_rho + r];
@@ -472,7 +499,10 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
                         __stcg(onlist + io, make_uint2(L, c));
                         __stcg(parent + L, tag | L);
                         __stcg(csize + L, 0u);
-                        if ((tl < P.S - 1 || last_strip) && is_peak<CW>(P, tile, halo, tl, r, c)) {
+                        // with theta_wrap, row 0 waits for the last row (tested after the strips) and the last row looks into row 0
+                        const int tg = base + tl;
+                        if ((tl < P.S - 1 || last_strip) && !(wrap && tg == 0) &&
+                            is_peak<CW>(P, tile, halo, tl, r, c, (wrap && tg == P.n_theta - 1) ? first_rows : nullptr)) {
                             const int i = atomicAdd(&sh.n_peaks, 1);
                             const uint2 rec = make_uint2(L, c);
                             if (i < P.PCAP) peaks_s[i] = rec; else __stcg(peaks_ovf + (i - P.PCAP), rec);
@@ -498,7 +528,32 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
             continue;
         }
 
-        // ---------------- S3: connected components of the on mask (8-connectivity, no wrap)
+        if (wrap && n_strips_e > 0) {
+            // theta row 0 (skipped above): the row before it is the last theta row mirrored, whose bins have the larger linear
+            // indices and lose ties; that row is still in the tile of the last strip
+            const int tl_last = P.n_theta - 1 - (P.n_strips - 1) * P.S;
+            for (int r = tid; r < P.n_rho; r += nthr) {
+                const uint32_t c = __ldcg(first_rows + r);
+                if (c < (uint32_t)P.T) continue;
+                bool pk = true;
+#pragma unroll
+                for (int dr = -1; dr <= 1; ++dr) {
+                    const int m = P.n_rho - 1 - (r + dr);
+                    if ((unsigned)m < (unsigned)P.n_rho && tile_get<CW>(tile, P.S, m, tl_last) > c) pk = false;
+                    if ((unsigned)(r + dr) < (unsigned)P.n_rho && __ldcg(first_rows + P.n_rho + r + dr) > c) pk = false;
+                }
+                if (r > 0 && __ldcg(first_rows + r - 1) >= c) pk = false;
+                if (r + 1 < P.n_rho && __ldcg(first_rows + r + 1) > c) pk = false;
+                if (pk) {
+                    const int i = atomicAdd(&sh.n_peaks, 1);
+                    const uint2 rec = make_uint2((uint32_t)r, c);
+                    if (i < P.PCAP) peaks_s[i] = rec; else __stcg(peaks_ovf + (i - P.PCAP), rec);
+                }
+            }
+            __syncthreads();
+        }
+
+        // ---------------- S3: connected components of the on mask (8-connectivity; across the theta seam only with theta_wrap)
         const int n_on = sh.n_on;
         const int n_pk = sh.n_peaks;
         for (int i = tid; i < n_on; i += nthr) {
@@ -511,6 +566,14 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
                 if ((__ldcg(parent + up) >> kLBits) == epoch) uf_union(parent, L, up, tag);
                 if (r > 0 && (__ldcg(parent + up - 1) >> kLBits) == epoch) uf_union(parent, L, up - 1, tag);
                 if (r + 1 < P.n_rho && (__ldcg(parent + up + 1) >> kLBits) == epoch) uf_union(parent, L, up + 1, tag);
+            } else if (wrap) {  // row 0 continues into the last theta row, rho mirrored; each pair across the seam is visited from here
+#pragma unroll
+                for (int dr = -1; dr <= 1; ++dr) {
+                    const int m = P.n_rho - 1 - (r + dr);
+                    if ((unsigned)m >= (unsigned)P.n_rho) continue;
+                    const uint32_t nb = (uint32_t)((P.n_theta - 1) * P.n_rho + m);
+                    if ((__ldcg(parent + nb) >> kLBits) == epoch) uf_union(parent, L, nb, tag);
+                }
             }
         }
         __syncthreads();

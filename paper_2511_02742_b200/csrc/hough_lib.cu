@@ -221,11 +221,15 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     if (d->max_candidates < 1 || d->max_candidates > 4096) return HOUGH_EINVAL;
     if (d->count_dtype != HOUGH_I32 && d->count_dtype != HOUGH_U16) return HOUGH_EINVAL;
     if (d->max_events < 1 || d->max_hits < 0 || d->max_hits_per_event < 0 || d->device < 0) return HOUGH_EINVAL;
-    if (d->flags & ~(HOUGH_FLAG_GENERAL_ONLY | HOUGH_FLAG_SMALL_LISTS)) return HOUGH_EINVAL;
+    if (d->flags & ~(HOUGH_FLAG_GENERAL_ONLY | HOUGH_FLAG_SMALL_LISTS | HOUGH_FLAG_THETA_WRAP)) return HOUGH_EINVAL;
     // theta window: (0, 0) = the paper's [0, pi)
     const bool th_default = d->theta_min == 0.0 && d->theta_max == 0.0;
     const double th_lo = d->theta_min, th_hi = th_default ? 3.14159265358979323846 : d->theta_max;
     if (!isfinite(th_lo) || !isfinite(th_hi) || !(th_hi > th_lo) || th_hi - th_lo > 6.283185307179586) return HOUGH_EINVAL;
+    // theta wrap (reading B9): row n_theta is row 0 with rho mirrored -- true only for [0, pi) and a rho range symmetric about 0
+    const bool theta_wrap = (d->flags & HOUGH_FLAG_THETA_WRAP) != 0;
+    if (theta_wrap && (!(th_default || (th_lo == 0.0 && th_hi == 3.14159265358979323846)) || d->rho_min != -d->rho_max || d->n_theta < 3))
+        return HOUGH_EINVAL;
     if (d->count_dtype == HOUGH_U16 && d->max_hits_per_event > 65535) return HOUGH_ERANGE;  // a bin gets <= 1 vote per hit
     if ((int64_t)d->n_theta * d->n_rho > (1ll << hough::kLBits)) return HOUGH_ERANGE;
     const int H = d->hit_frac_bits < 0 ? 6 : d->hit_frac_bits;
@@ -348,7 +352,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     FastLayout flay{};
     int f_S = 0, f_nstrips = 0, f_tile = 0, f_HB = 0, f_SLCAP = 0, f_PCAP = 0, f_ONCAP = 0, f_k = 0;
     if (cw == 2 && d->vote_threshold <= 1023 && K <= 1000 && d->max_hits_per_event >= 1 && !env_int("HOUGH_NO_FAST", 0) &&
-        !(d->flags & HOUGH_FLAG_GENERAL_ONLY) &&
+        !(d->flags & HOUGH_FLAG_GENERAL_ONLY) && !theta_wrap &&  // the fast kernel has no seam logic: wrap plans use the general kernel
         // the reachable-row bound of the fast kernel keeps u_q^2 + v_q^2 in 32 bits
         2.0 * (double)qmax * (double)qmax <= 4294967295.0) {
         struct Cand { int G, maxt, minb, threads, cps; };
@@ -394,7 +398,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     // ---- device memory
     const size_t n_bins = (size_t)d->n_theta * d->n_rho;
     const size_t tab = (size_t)n_strips * S;
-    const size_t per_cta = n_bins * 4 + n_bins * 4 + n_bins * 8 + (n_bins / 4 + 1) * 8 + 16;
+    const size_t per_cta = n_bins * 4 + n_bins * 4 + n_bins * 8 + (n_bins / 4 + 1) * 8 + (size_t)d->n_rho * 8 + 256 + 16;
     const size_t scratch_bytes = align_up(per_cta, 256) * p->n_ctas + 256;
     std::vector<int32_t> padc(tab, 0), pads(tab, 0);
     memcpy(padc.data(), p->h_cos.data(), sizeof(int32_t) * d->n_theta);
@@ -453,6 +457,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     P.max_hits_per_event = d->max_hits_per_event;
     P.rho_min = d->rho_min; P.d_rho = d_rho;
     P.theta_min = th_lo; P.theta_span = th_hi - th_lo;
+    P.theta_wrap = theta_wrap ? 1 : 0;
     P.Cq = p->d_cos; P.Sq = p->d_sin;
     P.off_hits = lay.off_hits; P.off_halo = lay.off_halo; P.off_peaks = lay.off_peaks;
     P.off_kept = lay.off_kept; P.off_kroot = lay.off_kroot; P.off_hist = lay.off_hist;
@@ -463,6 +468,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
         P.csize = reinterpret_cast<uint32_t*>(b);               b += align_up(n_bins * 4 * nc, 256);
         P.onlist = reinterpret_cast<uint2*>(b);                 b += align_up(n_bins * 8 * nc, 256);
         P.peaks_ovf = reinterpret_cast<uint2*>(b);              b += align_up((n_bins / 4 + 1) * 8 * nc, 256);
+        P.first_rows = reinterpret_cast<uint32_t*>(b);          b += align_up((size_t)d->n_rho * 8 * nc, 256);
         P.epoch = reinterpret_cast<uint32_t*>(b);
         if ((size_t)(b - static_cast<unsigned char*>(p->d_scratch)) + nc * 4 > scratch_bytes) { hough_plan_destroy(p); return HOUGH_ENOMEM; }
     }
@@ -825,6 +831,7 @@ int hough_find_tracks_peeloff(hough_plan_t* p, const float* d_u, const float* d_
     int rc = check_common(p, d_u, d_v, d_offsets, n_events);
     if (rc) return rc;
     if (!d_cands || !d_n_found || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_n_found & 3)) return HOUGH_EINVAL;
+    if (p->desc.flags & HOUGH_FLAG_THETA_WRAP) return HOUGH_EINVAL;  // the global maximum has no neighbours to wrap
     if (n_events == 0) return HOUGH_OK;
     if (!d_labels && p->desc.max_hits > 0) return HOUGH_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -852,6 +859,7 @@ int hough_find_two_stage(hough_plan_t* p, const float* d_u, const float* d_v, co
     if (rc) return rc;
     if (!d_cands || !d_n_found || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_n_found & 3)) return HOUGH_EINVAL;
     if (coarse_theta < 1 || coarse_rho < 1 || coarse_theta > p->desc.n_theta || coarse_rho > p->desc.n_rho) return HOUGH_EINVAL;
+    if (p->desc.flags & HOUGH_FLAG_THETA_WRAP) return HOUGH_EINVAL;  // the coarse grid has no seam logic
     hough::TwoStageParams Q;
     Q.c_theta = coarse_theta; Q.c_rho = coarse_rho;
     Q.nT = (p->desc.n_theta + coarse_theta - 1) / coarse_theta;

@@ -24,7 +24,7 @@ LIB_PATH = os.path.join(_HERE, "libhough.so")
 HOUGH_OK, HOUGH_EINVAL, HOUGH_ERANGE, HOUGH_ECUDA, HOUGH_ENOMEM = 0, -1, -2, -3, -4
 HOUGH_I32, HOUGH_U16 = 0, 1
 HOUGH_STATUS_EVENT_TOO_LONG, HOUGH_STATUS_BAD_OFFSETS, HOUGH_STATUS_INTERNAL = 1, 2, 4
-HOUGH_FLAG_GENERAL_ONLY, HOUGH_FLAG_SMALL_LISTS = 1, 2
+HOUGH_FLAG_GENERAL_ONLY, HOUGH_FLAG_SMALL_LISTS, HOUGH_FLAG_THETA_WRAP = 1, 2, 4
 
 # numpy view of hough_candidate_t (32 bytes)
 CANDIDATE_DTYPE = np.dtype([("theta_bin", "<i4"), ("rho_bin", "<i4"), ("votes", "<i4"), ("cluster_root", "<i4"),

@@ -44,7 +44,9 @@ def random_case(rng):
     lo, hi = 0.0, math.pi
     if rng.random() < 0.2:
         lo = float(rng.uniform(0, 2)); hi = lo + float(rng.uniform(0.2, 3.0))
-    p = D.Params(n_theta, n_rho, rho_min, rho_max, coord, T, w, K, H, -1, lo, hi)
+    # theta wrap (reading B9) wherever the seam closes: default window, symmetric rho range, three or more rows
+    wrap = bool(lo == 0.0 and hi == math.pi and shift == 0.0 and n_theta >= 3 and rng.random() < 0.5)
+    p = D.Params(n_theta, n_rho, rho_min, rho_max, coord, T, w, K, H, -1, lo, hi, wrap)
     try:
         D.constants(p)
         if D.default_frac_bits(p) < 1:
@@ -63,6 +65,10 @@ def random_case(rng):
                 n = int(rng.integers(2, 60))
                 uu = rng.uniform(-coord, coord, n) * 0.9
                 m, c = rng.uniform(-2, 2), rng.uniform(-coord, coord) * 0.5
+                if wrap and rng.random() < 0.5:                       # a near-vertical group: its ridge crosses the theta seam
+                    vv = rng.uniform(-coord, coord, n) * 0.9
+                    parts_v.append(vv); parts_u.append(np.clip(c + rng.uniform(-0.05, 0.05) * vv, -coord, coord))
+                    continue
                 parts_u.append(uu); parts_v.append(np.clip(m * uu + c, -coord, coord))
             n_noise = int(rng.choice([0, 5, 40, 300, 1500]))
             parts_u.append(rng.uniform(-coord, coord, n_noise)); parts_v.append(rng.uniform(-coord, coord, n_noise))
@@ -87,7 +93,7 @@ def main():
     a = ap.parse_args()
     rng = np.random.default_rng(a.seed)
     done = bad = 0
-    paths = {"fast": 0, "general": 0, "deferred": 0}
+    paths = {"fast": 0, "general": 0, "deferred": 0, "wrap": 0}
     while done < a.cases:
         case = random_case(rng)
         if case is None:
@@ -110,12 +116,13 @@ def main():
         done += 1
         paths["fast" if g["info"]["fast_groups"] else "general"] += 1
         paths["deferred"] += g["deferred"]
+        paths["wrap"] += int(p.theta_wrap)
         if not ok:
             bad += 1
             print("MISMATCH", p, "flags", flags, "dtype", dt, "hits", len(u), "offsets", offsets.tolist(),
                   "viol", g["emu_violations"], g["bounds_violations"], g["bounds_site"], g["status"], flush=True)
     print(f"fuzz seed {a.seed}: {done} cases, {bad} mismatches; plans with a fast kernel {paths['fast']}, without {paths['general']}, "
-          f"events handed over {paths['deferred']}")
+          f"events handed over {paths['deferred']}, theta-wrap plans {paths['wrap']}")
     return 1 if bad else 0
 
 

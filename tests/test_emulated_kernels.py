@@ -501,3 +501,78 @@ def test_general_kernel_epoch_tags_wrap():
     o = oracle_run(p, u, v, offsets, want_acc=False)
     assert_same(g, o, p)
     assert (o["n_found"] >= 1).mean() > 0.9
+
+
+# ----------------------------------------------------------------------------- theta wrap (reading B9)
+def seam_events(n_events, seed, coord=94.0):
+    """Events whose tracks are vertical or nearly so (theta within a few bins of 0 / pi: their ridges cross the seam) plus
+    ordinary tracks and noise."""
+    rng = np.random.default_rng(seed)
+    us, vs, offs = [], [], [0]
+    for e in range(n_events):
+        uu, vv = [], []
+        for k in range(int(rng.integers(1, 4))):                             # near-vertical: u = c + small slope * v
+            c, tilt = rng.uniform(-0.9 * coord, 0.9 * coord), rng.uniform(-0.06, 0.06) if k else rng.uniform(-0.01, 0.01)
+            v = rng.uniform(-190, 190, int(rng.integers(20, 48)) if k else 48)
+            uu.append(np.clip(c + tilt * v + rng.normal(0, 0.1, len(v)), -coord, coord)); vv.append(v)
+        for _ in range(int(rng.integers(0, 3))):                             # ordinary tracks
+            a, b = synth.ideal_track(rng.uniform(-1, 1), rng.uniform(-100, 100))
+            uu.append(a); vv.append(b)
+        n_noise = int(rng.integers(0, 60))
+        uu.append(rng.uniform(-coord, coord, n_noise)); vv.append(rng.uniform(-190, 190, n_noise))
+        uu, vv = np.concatenate(uu).astype(np.float32), np.concatenate(vv).astype(np.float32)
+        pm = rng.permutation(len(uu))
+        us.append(uu[pm]); vs.append(vv[pm]); offs.append(offs[-1] + len(uu))
+    return np.concatenate(us), np.concatenate(vs), np.array(offs, np.int64)
+
+
+@pytest.mark.parametrize("grid,dt,K,T", [((256, 256), E.HOUGH_U16, 128, 10), ((1024, 256), E.HOUGH_U16, 64, 10),
+                                        ((180, 1000), E.HOUGH_I32, 16, 4), ((45, 64), E.HOUGH_I32, 3, 10), ((3, 33), E.HOUGH_U16, 8, 10)],
+                         ids=["256x256_u16", "1024x256_several_strips", "180x1000_i32", "45x64_K3", "three_rows"])
+def test_theta_wrap_variant(grid, dt, K, T):
+    """HOUGH_FLAG_THETA_WRAP: peaks and clusters that see across the theta seam, against the oracle with theta_wrap, and the
+    same plan without the flag against the oracle without (the flag must change nothing else)."""
+    u, v, offsets = seam_events(6, seed=grid[0])
+    u = np.concatenate([u, np.zeros(0, np.float32)]); offsets = np.append(offsets, offsets[-1])    # an empty event at the end
+    crossed = 0
+    for wrap in (True, False):
+        p = std_params(grid[0], grid[1], T=T, K=K, theta_wrap=wrap)
+        g = E.run(p, u, v, offsets, dt, want_acc=False)
+        o = oracle_run(p, u, v, offsets, want_acc=False)
+        assert_same(g, o, p)
+        assert g["info"]["fast_groups"] == 0 or not wrap                    # wrap plans use the general kernel
+        if wrap:
+            o_plain = oracle_run(std_params(grid[0], grid[1], T=10, K=K), u, v, offsets, want_acc=False)
+            crossed = sum(int(o["n_found"][e] != o_plain["n_found"][e] or o["cands"][e].tobytes() != o_plain["cands"][e].tobytes())
+                          for e in range(len(offsets) - 1))
+    assert crossed >= (1 if grid[0] >= 45 else 0)                            # the seam really matters on these events
+
+
+def test_theta_wrap_is_rejected_where_the_seam_does_not_close():
+    ok = std_params(64, 64)
+    for bad in (dict(rho_min=-256.0, rho_max=300.0), dict(n_theta=2), dict(theta_min=0.0, theta_max=1.5)):
+        p = std_params(**{**dict(n_theta=64, n_rho=64), **bad})
+        d = E.Desc(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, 6, -1, 5, 2.0, 8, E.HOUGH_I32, 1, 10, 10, E.FLAG_THETA_WRAP, 0,
+                   *E.theta_window(p))
+        h = E.ctypes.c_void_p()
+        assert E.lib().hough_plan_create(E.ctypes.byref(d), E.ctypes.byref(h)) == -1
+    d = E.Desc(ok.n_theta, ok.n_rho, ok.rho_min, ok.rho_max, ok.coord_max, 6, -1, 5, 2.0, 8, E.HOUGH_I32, 1, 10, 10, E.FLAG_THETA_WRAP, 0, 0.0, 0.0)
+    h = E.ctypes.c_void_p()
+    assert E.lib().hough_plan_create(E.ctypes.byref(d), E.ctypes.byref(h)) == 0
+    z = E.DevBuf(np.zeros(4, np.float32)); off = E.DevBuf(np.array([0, 4], np.int64))
+    cands = E.DevBuf(np.zeros((1, 8), E.CAND_DTYPE)); nf = E.DevBuf(np.zeros(1, np.int32)); lab = E.DevBuf(np.zeros(4, np.int32))
+    L = E.lib()
+    L.hough_find_tracks_peeloff.argtypes = [E.ctypes.c_void_p] * 4 + [E.ctypes.c_int32] + [E.ctypes.c_void_p] * 4
+    L.hough_find_two_stage.argtypes = [E.ctypes.c_void_p] * 4 + [E.ctypes.c_int32] * 3 + [E.ctypes.c_void_p] * 3
+    assert L.hough_find_tracks_peeloff(h, z.ptr, z.ptr, off.ptr, 1, cands.ptr, nf.ptr, lab.ptr, None) == -1
+    assert L.hough_find_two_stage(h, z.ptr, z.ptr, off.ptr, 1, 4, 4, cands.ptr, nf.ptr, None) == -1
+    L.hough_plan_destroy(h)
+
+
+@pytest.mark.parametrize("seed,preempt,workers", [(11, 0, 1), (12, 64, 1), (13, 8, 4)])
+def test_theta_wrap_does_not_depend_on_the_schedule(seed, preempt, workers):
+    u, v, offsets = seam_events(8, seed=5)
+    p = std_params(256, 128, T=10, K=32, theta_wrap=True)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    E.configure(seed=seed, preempt_per_1024=preempt, workers=workers)
+    assert_same(E.run(p, u, v, offsets, E.HOUGH_U16, want_acc=False), o, p)

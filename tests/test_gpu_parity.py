@@ -18,6 +18,8 @@ INT_FIELDS = ("theta_bin", "rho_bin", "votes", "cluster_root", "cluster_nbins", 
 
 
 def make_plan(p: D.Params, n_events, n_hits, max_hpe, count_dtype=H.HOUGH_I32, flags=0):
+    if p.theta_wrap:
+        flags |= H.HOUGH_FLAG_THETA_WRAP
     return H.hough_plan_create(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.vote_threshold, p.assign_window,
                                p.max_candidates, max(1, n_events), max(0, n_hits), max_hpe, count_dtype,
                                p.hit_frac_bits, p.acc_frac_bits, 0, flags,
@@ -417,6 +419,54 @@ def test_restricted_theta_window():
         for e in range(200):
             k = min(int(o["n_found"][e]), p.max_candidates)
             assert g["cands"][e, :k].tobytes() == o["cands"][e, :k].tobytes()
+
+
+@pytest.mark.parametrize("grid,dt,K,T,n_events", [((256, 256), H.HOUGH_U16, 128, 10, 400), ((1024, 256), H.HOUGH_U16, 64, 10, 300),
+                                                 ((180, 1000), H.HOUGH_I32, 16, 4, 300), ((45, 64), H.HOUGH_I32, 3, 10, 400),
+                                                 ((3, 33), H.HOUGH_U16, 8, 10, 100)],
+                         ids=["256x256_u16", "1024x256_several_strips", "180x1000_i32", "45x64_K3", "three_rows"])
+def test_theta_wrap_variant(grid, dt, K, T, n_events):
+    """SURVEY.md 8(f) item 4, reading B9 (HOUGH_FLAG_THETA_WRAP): peaks and clusters that see across the theta seam, on events
+    whose near-vertical tracks put their ridges across it; every record and label against the oracle with theta_wrap."""
+    from test_emulated_kernels import seam_events
+    u, v, offsets = seam_events(n_events, seed=grid[0] + 1)
+    p = std_params(grid[0], grid[1], T=T, K=K, theta_wrap=True)
+    g = gpu_run(p, u, v, offsets, dt, want_acc=False)
+    o = oracle_run(p, u, v, offsets, want_acc=False)
+    assert_same(g, o, p)
+    assert g["info"]["fast_groups"] == 0                                     # wrap plans use the general kernel
+    for e in range(n_events):
+        k = min(int(o["n_found"][e]), p.max_candidates)
+        assert g["cands"][e, :k].tobytes() == o["cands"][e, :k].tobytes()
+    o_plain = oracle_run(std_params(grid[0], grid[1], T=T, K=K), u, v, offsets, want_acc=False)
+    differ = sum(o["cands"][e].tobytes() != o_plain["cands"][e].tobytes() for e in range(n_events))
+    assert differ >= (n_events // 10 if grid[0] >= 45 else 0)                # the seam matters on these events
+
+
+def test_theta_wrap_on_the_high_pileup_grid():
+    """The wrap variant on the events and the grid of config 3 (the benchmark workload)."""
+    from dataclasses import replace
+    wl = synth.workload(3)
+    b = synth.generate(wl, 0, 60)
+    p = replace(params_of(wl), theta_wrap=True)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    g = gpu_run(p, b.u, b.v, b.offsets, H.HOUGH_U16, want_acc=False)
+    assert_same(g, o, p)
+
+
+def test_theta_wrap_is_rejected_where_the_seam_does_not_close():
+    for bad in (dict(rho_min=-256.0, rho_max=300.0), dict(n_theta=2), dict(theta_min=0.0, theta_max=1.5)):
+        p = std_params(**{**dict(n_theta=64, n_rho=64, theta_wrap=True), **bad})
+        with pytest.raises(Exception):
+            make_plan(p, 1, 16, 16)
+    plan = make_plan(std_params(64, 64, theta_wrap=True), 1, 16, 16)
+    z = torch.zeros(4, dtype=torch.float32, device="cuda")
+    off = torch.tensor([0, 4], dtype=torch.int64, device="cuda")
+    with pytest.raises(Exception):
+        H.hough_find_tracks_peeloff(plan, z, z, off)
+    with pytest.raises(Exception):
+        H.hough_find_two_stage(plan, z, z, off, 4, 4)
+    H.hough_plan_destroy(plan)
 
 
 def test_general_kernel_epoch_tags_wrap():
