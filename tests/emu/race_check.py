@@ -32,7 +32,8 @@ ROOT = os.path.dirname(os.path.dirname(HERE))
 # one case per kernel and per hand-over path; the whole file takes about ten times longer
 DEFAULT_K = ("test_configs_bit_exact and (0-1 or 2-12 or 3-6) or test_concurrent_ctas or test_mixed_batch or test_refit_tracks "
              "or test_frontend_slice or test_frontend_feeds or test_peeloff_variant or test_two_stage_variant "
-             "or test_dense_workload or test_edge_set_as_one_ragged_batch or test_run_host_chunked")
+             "or test_dense_workload or test_edge_set_as_one_ragged_batch or test_run_host_chunked or test_theta_wrap_variant "
+             "or test_theta_wrap_does_not")
 
 
 BARRIER = "__syncthreads();  // all votes of the strip are in"
