@@ -26,9 +26,12 @@
  *   - Return value: HOUGH_OK (0) or a negative hough_status code.  Nothing throws or aborts across the ABI.
  *   - Data-dependent conditions are not errors: an event with more than K local maxima reports the
  *     untruncated count in n_found and writes only the first K records; invalid hits (non-finite, or
- *     |u| or |v| > coord_max) cast no votes and get label -1; an event longer than max_hits_per_event or
- *     with decreasing offsets is skipped (no candidates, labels -1) and sets a bit in the plan's device
- *     status word (hough_plan_status).
+ *     |u| or |v| > coord_max) cast no votes and get label -1; an event longer than max_hits_per_event
+ *     (HOUGH_STATUS_EVENT_TOO_LONG), with a negative or decreasing offset, or ending beyond the plan's max_hits
+ *     (HOUGH_STATUS_BAD_OFFSETS: its hits would lie outside buffers of that capacity) is skipped -- no candidates,
+ *     n_found 0, its hits never read -- and sets that bit in the plan's device status word (hough_plan_status).
+ *   - Records, counts and labels that a call takes as INPUT are caller data: a record that names no bin of the plan's
+ *     grid attracts no hit, a label beyond the event's kept records is ignored; neither is used as an index.
  */
 #ifndef HOUGH_H_
 #define HOUGH_H_
@@ -82,7 +85,7 @@ typedef struct {
     int32_t max_candidates;       /* K in [1, 4096]: records kept per event                                 */
     int32_t count_dtype;          /* HOUGH_I32 or HOUGH_U16                                                 */
     int32_t max_events;           /* capacity: events per call                                              */
-    int64_t max_hits;             /* capacity: hits per call                                                */
+    int64_t max_hits;             /* capacity: hits per call; the kernels never read u, v or labels at or beyond it */
     int32_t max_hits_per_event;   /* capacity: hits in one event (HOUGH_U16 needs <= 65535).  Size it to the
                                      workload: the fast kernel stages this many hits in shared memory, at the
                                      cost of its other per-event lists (events that overflow those are still
@@ -144,8 +147,9 @@ int hough_find_clusters(hough_plan_t* plan, const float* d_u, const float* d_v, 
 /* Hit-to-candidate assignment: label[h] = slot of the kept candidate whose bin-centre line is
  * nearest to hit h (fixed-point residual at the candidate's theta), among those within the window; ties go to
  * the lower slot; -1 if none or if the hit is invalid.
- *   d_cands, d_n_found   as written by hough_find_clusters for the same events
- *   d_labels             [N] int32, every element of the events' ranges is written */
+ *   d_cands, d_n_found   as written by hough_find_clusters for the same events (16- and 4-byte aligned)
+ *   d_labels             [N] int32, every element of the events' ranges is written (skipped events: untouched); may be NULL
+ *                        only for a plan with max_hits = 0 */
 int hough_assign_hits(hough_plan_t* plan, const float* d_u, const float* d_v, const int64_t* d_offsets,
                       int32_t n_events, const hough_candidate_t* d_cands, const int32_t* d_n_found,
                       int32_t* d_labels, void* stream);

@@ -281,7 +281,7 @@ hough_fast_kernel(const DevParams P, const float* __restrict__ u, const float* _
             if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
             continue;
         }
-        if (!fold_ok || g0 < 0 || ne64 < 0 || ne64 > (long long)P.fHB || ne64 > (long long)P.max_hits_per_event) {
+        if (!fold_ok || g0 < 0 || ne64 < 0 || g1 > P.max_hits || ne64 > (long long)P.fHB || ne64 > (long long)P.max_hits_per_event) {
             // bad offsets, or more hits than the staging buffer: the general kernel handles (and flags) it
             if (tid == 0) P.deferred[atomicAdd(P.deferred_count, 1u)] = e;
             continue;

@@ -64,6 +64,7 @@ struct DevParams {
     int S, n_strips, row_bytes, tile_bytes;  // strip rows, strips per event, bytes per rho row of the tile
     int HB, PCAP;                            // capacity of the staged-hit buffer / the in-smem peak list
     int max_hits_per_event;
+    long long max_hits;  // the plan's hit capacity: an event that ends beyond it has bad offsets (its hits would be read out of range)
     double rho_min, d_rho;
     double theta_min, theta_span;  // theta_t = theta_min + theta_span t / n_theta
     const int* Cq;  // [n_strips * S], zero padded
@@ -372,7 +373,7 @@ hough_event_kernel(const DevParams P, const float* __restrict__ u, const float* 
         const long long g0 = offsets[e], g1 = offsets[e + 1];
         long long ne64 = g1 - g0;
         bool skip = false;
-        if (g0 < 0 || ne64 < 0) { if (tid == 0) atomicOr(P.status, 2); skip = true; }
+        if (g0 < 0 || ne64 < 0 || g1 > P.max_hits) { if (tid == 0) atomicOr(P.status, 2); skip = true; }
         else if (ne64 > (long long)P.max_hits_per_event) { if (tid == 0) atomicOr(P.status, 1); skip = true; }
         const int ne = skip ? 0 : (int)ne64;
         const int n_chunks = (ne + P.HB - 1) / P.HB;
@@ -706,7 +707,7 @@ hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float*
     const int tid = threadIdx.x, nthr = blockDim.x;
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
         const long long g0 = offsets[e], g1 = offsets[e + 1];
-        if (g0 < 0 || g1 < g0) continue;  // flagged by the find kernel
+        if (g0 < 0 || g1 < g0 || g1 > P.max_hits) continue;  // flagged by the find kernel
         const bool too_long = (g1 - g0) > (long long)P.max_hits_per_event;
         const int nk = too_long ? 0 : min(n_found[e], P.K);
         __syncthreads();
@@ -714,7 +715,10 @@ hough_assign_kernel(const DevParams P, const float* __restrict__ u, const float*
             const Candidate* c = cands + (size_t)e * P.K + s;
             const int t = c->theta_bin, r = c->rho_bin;
             const int half = P.F >= 1 ? (1 << (P.F - 1)) : 0;
-            trip[s] = make_int4(__ldg(P.Cq + t), __ldg(P.Sq + t), P.Oq - (r << P.F) - half, s);
+            // records are caller data: one that names no bin of this plan (not written by hough_find_clusters of the same plan)
+            // must not index the tables; it becomes a line no hit can reach (e = 2^31 - 1 > W_q for every hit)
+            const bool in_grid = (unsigned)t < (unsigned)P.n_theta && (unsigned)r < (unsigned)P.n_rho;
+            trip[s] = in_grid ? make_int4(__ldg(P.Cq + t), __ldg(P.Sq + t), P.Oq - (r << P.F) - half, s) : make_int4(0, 0, 0x7fffffff, s);
         }
         __syncthreads();
         // HPT hits per thread and trip: one broadcast load of a candidate triple serves HPT residuals.  best starts at

@@ -455,6 +455,7 @@ int hough_plan_create(const hough_plan_desc_t* d, hough_plan_t** out)
     P.S = S; P.n_strips = n_strips; P.row_bytes = 128 * G; P.tile_bytes = tile_bytes;
     P.HB = HB; P.PCAP = PCAP;
     P.max_hits_per_event = d->max_hits_per_event;
+    P.max_hits = d->max_hits;
     P.rho_min = d->rho_min; P.d_rho = d_rho;
     P.theta_min = th_lo; P.theta_span = th_hi - th_lo;
     P.theta_wrap = theta_wrap ? 1 : 0;
@@ -614,7 +615,9 @@ int hough_assign_hits(hough_plan_t* p, const float* d_u, const float* d_v, const
     int rc = check_common(p, d_u, d_v, d_offsets, n_events);
     if (rc) return rc;
     if (!d_cands || !d_n_found) return HOUGH_EINVAL;
+    if (((uintptr_t)d_cands & 15) || ((uintptr_t)d_n_found & 3) || ((uintptr_t)d_labels & 3)) return HOUGH_EINVAL;
     if (n_events == 0) return HOUGH_OK;
+    if (!d_labels && p->desc.max_hits > 0) return HOUGH_EINVAL;  // only a plan without hits has nothing to label
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     HCK(cudaSetDevice(p->desc.device));
     const int grid = n_events < p->assign_ctas ? n_events : p->assign_ctas;

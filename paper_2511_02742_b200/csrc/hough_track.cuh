@@ -201,14 +201,14 @@ hough_refit_kernel(const DevParams P, const PlaneParams G, const float* __restri
     const int tid = threadIdx.x, nthr = blockDim.x;
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
         const long long g0 = offsets[e], g1 = offsets[e + 1];
-        if (g0 < 0 || g1 < g0 || (g1 - g0) > (long long)P.max_hits_per_event) continue;  // flagged by the find kernel: no records
+        if (g0 < 0 || g1 < g0 || g1 > P.max_hits || (g1 - g0) > (long long)P.max_hits_per_event) continue;  // flagged by the find kernel: no records
         const int nk = min(max(n_found[e], 0), P.K);
         __syncthreads();  // the previous event's records are written
         for (int s = tid; s < nk; s += nthr) acc[s] = FitAcc{0ull, 0ull, 0ull, 0ull, 0ull, 0u, 0u};
         __syncthreads();
         for (long long i = g0 + tid; i < g1; i += nthr) {
             const int lab = labels[i];
-            if (lab < 0 || !HB(P, lab, nk, 310)) continue;  // unassigned or invalid hit
+            if (lab < 0 || lab >= nk) continue;  // unassigned or invalid hit; labels are caller data: one beyond the kept records is ignored
             const int uq = __float2int_rn(__ldg(u + i) * P.hit_scale), vq = __float2int_rn(__ldg(v + i) * P.hit_scale);
             FitAcc& A = acc[lab];
             atomicAdd(&A.n, 1u);
@@ -271,9 +271,10 @@ hough_peel_kernel(const DevParams P, int S, const float* __restrict__ u, const f
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
         const long long g0 = offsets[e], g1 = offsets[e + 1];
         __syncthreads();
-        if (g0 < 0 || g1 < g0 || (g1 - g0) > (long long)P.max_hits_per_event) {
-            if (tid == 0) { atomicOr(P.status, (g0 < 0 || g1 < g0) ? 2 : 1); n_found[e] = 0; }
-            if (g0 >= 0 && g1 >= g0) for (long long i = g0 + tid; i < g1; i += nthr) labels[i] = -1;
+        const bool bad_offsets = g0 < 0 || g1 < g0 || g1 > P.max_hits;
+        if (bad_offsets || (g1 - g0) > (long long)P.max_hits_per_event) {
+            if (tid == 0) { atomicOr(P.status, bad_offsets ? 2 : 1); n_found[e] = 0; }
+            if (!bad_offsets) for (long long i = g0 + tid; i < g1; i += nthr) labels[i] = -1;
             continue;
         }
         const int ne = (int)(g1 - g0);
@@ -392,8 +393,9 @@ hough_two_stage_kernel(const DevParams P, const TwoStageParams Q, const float* _
     for (int e = blockIdx.x; e < n_events; e += gridDim.x) {
         const long long g0 = offsets[e], g1 = offsets[e + 1];
         __syncthreads();
-        if (g0 < 0 || g1 < g0 || (g1 - g0) > (long long)P.max_hits_per_event) {
-            if (tid == 0) { atomicOr(P.status, (g0 < 0 || g1 < g0) ? 2 : 1); n_found[e] = 0; }
+        const bool bad_offsets = g0 < 0 || g1 < g0 || g1 > P.max_hits;
+        if (bad_offsets || (g1 - g0) > (long long)P.max_hits_per_event) {
+            if (tid == 0) { atomicOr(P.status, bad_offsets ? 2 : 1); n_found[e] = 0; }
             continue;
         }
         const int ne = (int)(g1 - g0);

@@ -149,6 +149,29 @@ def run(p, u, v, offsets, count_dtype=HOUGH_I32, want_acc=True, max_hpe=None, fl
     return out
 
 
+def assign(p, u, v, offsets, cands, n_found, count_dtype=HOUGH_I32):
+    """hough_assign_hits alone, on caller-made records (cands [E][K] of CAND_DTYPE, n_found [E]) -> (labels, return code)."""
+    L = lib()
+    L.cuda_emu_reset_violations()
+    E = len(offsets) - 1
+    hpe = int(np.diff(offsets).max()) if E > 0 and len(u) else 0
+    d = Desc(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.hit_frac_bits, p.acc_frac_bits, p.vote_threshold,
+             p.assign_window, p.max_candidates, count_dtype, max(1, E), max(0, len(u)), max(hpe, 1), 0, 0, *theta_window(p))
+    h = ctypes.c_void_p()
+    assert L.hough_plan_create(ctypes.byref(d), ctypes.byref(h)) == 0
+    du, dv, do = DevBuf(np.asarray(u, np.float32)), DevBuf(np.asarray(v, np.float32)), DevBuf(np.asarray(offsets, np.int64))
+    dc, dn = DevBuf(np.ascontiguousarray(cands, CAND_DTYPE)), DevBuf(np.asarray(n_found, np.int32))
+    labels = DevBuf(np.full(len(u), -99, np.int32))
+    rc = L.hough_assign_hits(h, du.ptr, dv.ptr, do.ptr, E, dc.ptr, dn.ptr, labels.ptr, None)
+    rc_null = L.hough_assign_hits(h, du.ptr, dv.ptr, do.ptr, E, dc.ptr, dn.ptr, None, None)
+    dbg = np.zeros(16, np.uint64)
+    L.hough_plan_debug_counters(h, dbg.ctypes.data, None)
+    L.hough_plan_destroy(h)
+    assert L.cuda_emu_violations() == 0, L.cuda_emu_first_violation().decode()
+    assert int(dbg[14]) == 0, f"index check failed at site {int(dbg[13])}"
+    return labels.view.copy(), rc, rc_null
+
+
 def run_host(p, u, v, offsets, n_chunks, count_dtype=HOUGH_I32, repeat=1):
     """hough_run_host_chunked on the emulated device (called `repeat` times on one plan; the last results are returned)."""
     L = lib()

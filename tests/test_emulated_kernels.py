@@ -576,3 +576,76 @@ def test_theta_wrap_does_not_depend_on_the_schedule(seed, preempt, workers):
     o = oracle_run(p, u, v, offsets, want_acc=False)
     E.configure(seed=seed, preempt_per_1024=preempt, workers=workers)
     assert_same(E.run(p, u, v, offsets, E.HOUGH_U16, want_acc=False), o, p)
+
+
+# ----------------------------------------------------------------------------- caller data that names nothing of the plan
+def test_assign_ignores_records_that_name_no_bin_of_the_plan():
+    """hough_assign_hits on records the caller made up: slots whose (theta_bin, rho_bin) lie outside the grid must not index the
+    tables (on the GPU: an out-of-range read); they attract no hit, and the good slots label exactly as the oracle says."""
+    wl = synth.workload(1)
+    b = synth.generate(wl, 0, 6)
+    p = params_of(wl)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    cands = o["cands"].copy()
+    n_found = o["n_found"].copy()
+    bad_slots = {}
+    for e in range(6):
+        nk = min(int(n_found[e]), p.max_candidates)
+        if nk >= 2:
+            s = nk - 1                                                       # the last kept record becomes garbage
+            cands[e, s]["theta_bin"], cands[e, s]["rho_bin"] = [(-1, 5), (p.n_theta, 0), (3, -7), (2 ** 30, 2 ** 30), (0, p.n_rho), (-2 ** 31, 1)][e]
+            bad_slots[e] = s
+    assert bad_slots
+    labels, rc, rc_null = E.assign(p, b.u, b.v, b.offsets, cands, n_found)
+    assert rc == 0 and rc_null == -1                                         # a null labels pointer is refused, not written through
+    for e in range(6):
+        a, z = int(b.offsets[e]), int(b.offsets[e + 1])
+        nk = min(int(n_found[e]), p.max_candidates)
+        good = [c for s, c in enumerate(o["cands"][e, :nk]) if s != bad_slots.get(e)]
+        want = C.assign_event(b.u[a:z], b.v[a:z], np.array(good, C.CAND_DTYPE), p)   # slots keep their numbers: the bad one is the last
+        np.testing.assert_array_equal(labels[a:z], want)
+        assert bad_slots.get(e, -5) not in set(labels[a:z].tolist())
+
+
+def test_refit_ignores_labels_beyond_the_kept_records():
+    wl = synth.workload(1)
+    b = synth.generate(wl, 0, 5)
+    p = params_of(wl)
+    o = C.run_batch(b.u, b.v, b.offsets, p)
+    labels = o["labels"].copy()
+    labels[::7] = np.array([p.max_candidates, 2 ** 30, 99, 4096], np.int32)[np.arange(len(labels[::7])) % 4]   # made-up slots
+    fits, rc = E.refit(p, b.u, b.v, b.offsets, o["n_found"], labels, GEOM)
+    assert rc == 0
+    for e in range(5):
+        a, z = int(b.offsets[e]), int(b.offsets[e + 1])
+        nk = min(int(o["n_found"][e]), p.max_candidates)
+        lab = labels[a:z].copy()
+        lab[lab >= nk] = -1                                                  # what "ignored" means
+        fits_equal(fits[e], T.refit_event(b.u[a:z], b.v[a:z], lab, nk, p, GEOM))
+
+
+@pytest.mark.parametrize("flags", [0, E.FLAG_GENERAL_ONLY], ids=["fast", "general_only"])
+def test_an_event_that_ends_beyond_the_plans_hit_capacity_is_flagged_not_read(flags):
+    """offsets[e + 1] > max_hits: the hits of that event would be read past the caller's buffers (the model ends them at an
+    inaccessible page).  The event is flagged BAD_OFFSETS and skipped by every kernel; its neighbours are computed."""
+    wl = synth.workload(1)
+    b = synth.generate(wl, 0, 3)
+    p = params_of(wl)
+    n = len(b.u)
+    offsets = b.offsets.copy()
+    offsets[3] = n + 50                                                      # the last event claims 50 hits that do not exist
+    g = E.run(p, b.u, b.v, offsets, flags=flags, want_vote=False)           # E.run sizes the plan by len(u): max_hits = n
+    assert g["emu_violations"] == 0 and g["bounds_violations"] == 0
+    assert g["status"] == 2
+    o = C.run_batch(b.u, b.v, b.offsets, p)
+    np.testing.assert_array_equal(g["n_found"][:2], o["n_found"][:2])
+    assert g["n_found"][2] == 0
+    a = int(b.offsets[2])
+    np.testing.assert_array_equal(g["labels"][:a], o["labels"][:a])
+    assert (g["labels"][a:] == -99).all()                                    # untouched
+    fits, rc = E.refit(p, b.u, b.v, offsets, g["n_found"], np.where(g["labels"] == -99, -1, g["labels"]), GEOM)
+    assert rc == 0 and (fits[2]["n_hits"] == 0).all()
+    pe = E.peeloff(std_params(64, 64, T=8, K=4), b.u, b.v, offsets, max_hpe=int(np.diff(offsets).max()))
+    assert pe["status"] == 2 and pe["n_found"][2] == 0
+    ts = E.two_stage(std_params(64, 64, T=8, K=4), b.u, b.v, offsets, 4, 4)
+    assert ts["rc"] == 0 and ts["n_found"][2] == 0

@@ -352,6 +352,59 @@ def test_status_word_flags_long_events_and_bad_offsets():
     np.testing.assert_array_equal(g["labels"][:50], o["labels"])
 
 
+def test_an_event_that_ends_beyond_the_plans_hit_capacity_is_flagged_not_read():
+    """offsets[e + 1] > max_hits: BAD_OFFSETS, the event is skipped by every kernel (its hits would lie past the buffers)."""
+    wl = synth.workload(1)
+    b = synth.generate(wl, 0, 3)
+    p = params_of(wl)
+    n = len(b.u)
+    offsets = b.offsets.copy()
+    offsets[3] = n + 50
+    o = C.run_batch(b.u, b.v, b.offsets, p)
+    a = int(b.offsets[2])
+    for flags in (0, H.HOUGH_FLAG_GENERAL_ONLY):
+        plan = make_plan(p, 3, n, int(np.diff(offsets).max()), H.HOUGH_I32, flags)        # max_hits = n
+        du, dv = torch.from_numpy(b.u).cuda(), torch.from_numpy(b.v).cuda()
+        do = torch.from_numpy(offsets).cuda()
+        cands, n_found = H.hough_find_clusters(plan, du, dv, do)
+        labels = torch.full((n,), -99, dtype=torch.int32, device="cuda")
+        H.hough_assign_hits(plan, du, dv, do, cands, n_found, labels=labels)
+        torch.cuda.synchronize()
+        assert H.hough_plan_status(plan) == H.HOUGH_STATUS_BAD_OFFSETS
+        nf, lab = n_found.cpu().numpy(), labels.cpu().numpy()
+        np.testing.assert_array_equal(nf[:2], o["n_found"][:2])
+        assert nf[2] == 0 and (lab[a:] == -99).all()
+        np.testing.assert_array_equal(lab[:a], o["labels"][:a])
+        H.hough_plan_destroy(plan)
+
+
+def test_assign_ignores_records_that_name_no_bin_of_the_plan():
+    """Records are caller data: slots whose bin lies just outside the grid must not index the tables and attract no hit."""
+    wl = synth.workload(1)
+    b = synth.generate(wl, 0, 6)
+    p = params_of(wl)
+    o = oracle_run(p, b.u, b.v, b.offsets, want_acc=False)
+    cands = o["cands"].copy()
+    bad_slots = {}
+    for e in range(6):
+        nk = min(int(o["n_found"][e]), p.max_candidates)
+        if nk >= 2:
+            cands[e, nk - 1]["theta_bin"], cands[e, nk - 1]["rho_bin"] = [(-1, 5), (p.n_theta, 0), (3, -7), (1, p.n_rho), (0, p.n_rho + 3), (-2, 1)][e]
+            bad_slots[e] = nk - 1
+    assert bad_slots
+    plan = make_plan(p, 6, len(b.u), int(np.diff(b.offsets).max()))
+    du, dv, do = torch.from_numpy(b.u).cuda(), torch.from_numpy(b.v).cuda(), torch.from_numpy(b.offsets).cuda()
+    dc = torch.from_numpy(np.ascontiguousarray(cands).view(np.int32).reshape(6, p.max_candidates, 8)).cuda()
+    dn = torch.from_numpy(o["n_found"]).cuda()
+    labels = H.hough_assign_hits(plan, du, dv, do, dc, dn).cpu().numpy()
+    H.hough_plan_destroy(plan)
+    for e in range(6):
+        a, z = int(b.offsets[e]), int(b.offsets[e + 1])
+        nk = min(int(o["n_found"][e]), p.max_candidates)
+        good = np.array([c for s, c in enumerate(o["cands"][e, :nk]) if s != bad_slots.get(e)], C.CAND_DTYPE)
+        np.testing.assert_array_equal(labels[a:z], C.assign_event(b.u[a:z], b.v[a:z], good, p))
+
+
 @pytest.mark.parametrize("n_chunks,n_events", [(0, 32), (1, 32), (3, 500), (7, 500), (32, 40)])
 def test_run_host_chunked_equals_oracle(n_chunks, n_events):
     """hough_run_host / hough_run_host_chunked: the three-stream chunk pipeline (upload, compute, download), called twice on

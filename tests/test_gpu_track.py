@@ -110,6 +110,29 @@ def check_refit(cfg, n_events, geom):
         assert (fits[e, nk:]["n_hits"] == 0).all()
 
 
+def test_refit_ignores_labels_beyond_the_kept_records():
+    """Labels are caller data: one that names no kept record of its event must not index the per-candidate sums."""
+    from test_emulated_kernels import fits_equal, GEOM
+    wl = synth.workload(1)
+    b = synth.generate(wl, 0, 5)
+    p = params_of(wl)
+    o = C.run_batch(b.u, b.v, b.offsets, p)
+    labels = o["labels"].copy()
+    labels[::7] = np.array([p.max_candidates, p.max_candidates + 1, 99, 130], np.int32)[np.arange(len(labels[::7])) % 4]
+    plan = H.hough_plan_create(p.n_theta, p.n_rho, p.rho_min, p.rho_max, p.coord_max, p.vote_threshold, p.assign_window,
+                               p.max_candidates, 5, len(b.u), int(np.diff(b.offsets).max()))
+    fits = H.fits_to_numpy(H.hough_refit_tracks(plan, torch.from_numpy(b.u).cuda(), torch.from_numpy(b.v).cuda(),
+                                                torch.from_numpy(b.offsets).cuda(), torch.from_numpy(o["n_found"]).cuda(),
+                                                torch.from_numpy(labels).cuda(), GEOM.origin, GEOM.pitch, GEOM.n_planes))
+    H.hough_plan_destroy(plan)
+    for e in range(5):
+        a, z = int(b.offsets[e]), int(b.offsets[e + 1])
+        nk = min(int(o["n_found"][e]), p.max_candidates)
+        lab = labels[a:z].copy()
+        lab[lab >= nk] = -1
+        fits_equal(fits[e], T.refit_event(b.u[a:z], b.v[a:z], lab, nk, p, GEOM))
+
+
 def test_refit_rejects_plans_whose_sums_could_overflow():
     plan = H.hough_plan_create(64, 512, -1415.0, 1415.0, 1000.0, 3, 6.0, 16, 1, 4, 4)
     z4 = torch.zeros(4, device="cuda")
