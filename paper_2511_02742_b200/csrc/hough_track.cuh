@@ -37,7 +37,7 @@ struct FrontParams {
 // phi = atan2(y, x) in units of 2^-16 degree: integer CORDIC, vectoring mode (reading B2).  (xq, yq) != (0, 0), |xq|, |yq| <= 2^15.
 __device__ __forceinline__ int cordic_phi_q(const FrontParams& FP, int xq, int yq)
 {
-    int X = abs(xq) << kCordicGuard, Y = yq << kCordicGuard, Z = 0;
+    int X = abs(xq) << kCordicGuard, Y = yq * (1 << kCordicGuard), Z = 0;  // (a left shift of a negative value is undefined before C++20)
 #pragma unroll
     for (int i = 0; i < kCordicIters; ++i) {
         const int xs = X >> i, ys = Y >> i;  // arithmetic shifts: floor

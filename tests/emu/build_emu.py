@@ -2,7 +2,7 @@
 the host CUDA model of cuda_emu.h.  TEST INFRASTRUCTURE -- NOT PART OF THE PRODUCT (nothing under paper_2511_02742_b200/
 imports or loads it).
 
-    python tests/emu/build_emu.py [--force] [--tsan]
+    python tests/emu/build_emu.py [--force] [--tsan | --ubsan]
 
 --tsan builds tests/emu/libhough_emu_tsan.so, the race-detector variant: the kernel sources are compiled with
 -fsanitize=thread and -DHOUGH_EMU_TSAN (every CUDA thread a ThreadSanitizer fiber, see cuda_emu.cpp); the model itself
@@ -44,6 +44,23 @@ def build_tsan(force: bool = False, csrc: str = _CSRC, out: str = LIB_TSAN) -> s
     return out
 
 
+LIB_UBSAN = os.path.join(_HERE, "libhough_emu_ubsan.so")
+
+
+def build_ubsan(force: bool = False) -> str:
+    """The host model with -fsanitize=undefined: shift counts >= the width (x86 masks them, the GPU clamps them -- a place
+    where the model and the hardware would silently differ), signed overflow, misaligned vector accesses.  Run with
+    LD_PRELOAD=$(gcc -print-file-name=libubsan.so) HOUGH_EMU_LIB=tests/emu/libhough_emu_ubsan.so UBSAN_OPTIONS=log_path=..."""
+    if not force and os.path.exists(LIB_UBSAN) and all(os.path.getmtime(d) <= os.path.getmtime(LIB_UBSAN) for d in DEPENDS):
+        return LIB_UBSAN
+    tmp = LIB_UBSAN + f".tmp{os.getpid()}"
+    subprocess.check_call(["g++", "-std=c++17", "-O1", "-g", "-fPIC", "-shared", "-ffp-contract=off", "-fno-strict-aliasing", "-DHOUGH_EMU",
+                           "-DHOUGH_BOUNDS", "-fsanitize=undefined", "-fno-sanitize=vptr", "-Wno-unknown-pragmas", "-I", _HERE, "-x", "c++",
+                           os.path.join(_CSRC, "hough_lib.cu"), os.path.join(_HERE, "cuda_emu.cpp"), "-o", tmp, "-pthread"])
+    os.replace(tmp, LIB_UBSAN)
+    return LIB_UBSAN
+
+
 def build(force: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(d) <= os.path.getmtime(LIB) for d in DEPENDS):
         return LIB
@@ -58,4 +75,4 @@ def build(force: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print((build_tsan if "--tsan" in sys.argv else build)(force="--force" in sys.argv))
+    print((build_tsan if "--tsan" in sys.argv else build_ubsan if "--ubsan" in sys.argv else build)(force="--force" in sys.argv))
