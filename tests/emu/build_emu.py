@@ -55,7 +55,7 @@ def build_ubsan(force: bool = False) -> str:
         return LIB_UBSAN
     tmp = LIB_UBSAN + f".tmp{os.getpid()}"
     subprocess.check_call(["g++", "-std=c++17", "-O1", "-g", "-fPIC", "-shared", "-ffp-contract=off", "-fno-strict-aliasing", "-DHOUGH_EMU",
-                           "-DHOUGH_BOUNDS", "-fsanitize=undefined", "-fno-sanitize=vptr", "-Wno-unknown-pragmas", "-I", _HERE, "-x", "c++",
+                           "-DHOUGH_BOUNDS", "-fsanitize=undefined,float-cast-overflow", "-fno-sanitize=vptr", "-Wno-unknown-pragmas", "-I", _HERE, "-x", "c++",
                            os.path.join(_CSRC, "hough_lib.cu"), os.path.join(_HERE, "cuda_emu.cpp"), "-o", tmp, "-pthread"])
     os.replace(tmp, LIB_UBSAN)
     return LIB_UBSAN
