@@ -708,6 +708,11 @@ int hough_run_host_chunked(hough_plan_t* p, const float* h_u, const float* h_v, 
     if (n_chunks > n_events) n_chunks = n_events;
     const size_t K = (size_t)p->desc.max_candidates;
     cudaStream_t st = p->h_stream;
+    // an error return in the middle of the batch first waits for the copies already queued: they read and write the caller's buffers
+    auto drain = [&](int rc) {
+        cudaStreamSynchronize(p->h_up); cudaStreamSynchronize(st); cudaStreamSynchronize(p->h_down);
+        return rc;
+    };
     HCK(cudaMemcpyAsync(p->hd_off, h_offsets, (size_t)(n_events + 1) * 8, cudaMemcpyHostToDevice, p->h_up));
     int e0 = 0;
     for (int c = 0; c < n_chunks; ++c) {
@@ -720,7 +725,7 @@ int hough_run_host_chunked(hough_plan_t* p, const float* h_u, const float* h_v, 
         }
         const int ne = e1 - e0;
         const int64_t a = h_offsets[e0], z = h_offsets[e1];
-        if (z < a || a < 0 || z > n_hits) return HOUGH_EINVAL;  // offsets must be non-decreasing on this path
+        if (z < a || a < 0 || z > n_hits) return drain(HOUGH_EINVAL);  // offsets must be non-decreasing on this path
         if (z > a) {
             HCK(cudaMemcpyAsync(p->hd_u + a, h_u + a, (size_t)(z - a) * 4, cudaMemcpyHostToDevice, p->h_up));
             HCK(cudaMemcpyAsync(p->hd_v + a, h_v + a, (size_t)(z - a) * 4, cudaMemcpyHostToDevice, p->h_up));
@@ -730,12 +735,12 @@ int hough_run_host_chunked(hough_plan_t* p, const float* h_u, const float* h_v, 
         if (ne > 0) {
             int rc = hough_find_clusters(p, p->hd_u, p->hd_v, reinterpret_cast<const int64_t*>(p->hd_off) + e0, ne,
                                          reinterpret_cast<hough_candidate_t*>(p->hd_cands) + (size_t)e0 * K, p->hd_nfound + e0, st);
-            if (rc) return rc;
+            if (rc) return drain(rc);
             if (h_labels) {
                 rc = hough_assign_hits(p, p->hd_u, p->hd_v, reinterpret_cast<const int64_t*>(p->hd_off) + e0, ne,
                                        reinterpret_cast<const hough_candidate_t*>(p->hd_cands) + (size_t)e0 * K, p->hd_nfound + e0,
                                        p->hd_labels, st);
-                if (rc) return rc;
+                if (rc) return drain(rc);
             }
         }
         HCK(cudaEventRecord(p->h_ev_done[c], st));
