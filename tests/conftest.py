@@ -31,3 +31,10 @@ def pytest_collection_modifyitems(config, items):
         for it in items:
             if "gate" not in it.keywords:
                 it.add_marker(skip)
+    # small before large: among the GPU tests the gate cases (<= 8 events each) run first, so that under -x a build
+    # that is wrong fails on a handful of events before anything is launched at full size.  The sort is stable: everything else
+    # (and every CPU test) keeps its place relative to its peers.
+    gpu_positions = [i for i, it in enumerate(items) if "gpu" in it.keywords]
+    gpu_items = sorted((items[i] for i in gpu_positions), key=lambda it: 0 if "gate" in it.keywords else 1)
+    for i, it in zip(gpu_positions, gpu_items):
+        items[i] = it
