@@ -15,6 +15,8 @@ What it computes (per event, independently), with the passage each step follows:
                 all strict local maxima >= threshold                BASELINE.json north_star, reading A7
   O5 clusters   8-connected components of the thresholded mask      PAPER.md L29 keyword "cluster finding",
                                                                     reading A7
+     (option theta_wrap, reading B9: O4 and O5 on the neighbourhood that continues past the theta seam -- the line
+      (theta + pi, rho) is the line (theta, -rho), Eq. 4.1; pinned by P9w, brute force on the unrolled theta axis)
   O6 rank       order by (votes desc, index asc), keep K            reading A8/A11
   O7 assign     "selecting the hits that align with the straight    PAPER.md L106, L94; reading A12/A13
                 line formed by the identified (theta, rho)"

@@ -15,6 +15,8 @@
  *   O4 peaks      PAPER.md L94/L106 "bin with the highest number of entries", generalised to every strict
  *                 local maximum >= T under the total order (count, -index)                    (A7/A8)
  *   O5 clusters   8-connected components of the thresholded mask (keyword L29)                (A7)
+ *                 theta_wrap != 0 (reading B9): O4 / O5 on the neighbourhood that continues past the theta seam,
+ *                 row n_theta = row 0 with rho mirrored (Eq. 4.1: (theta + pi, rho) = (theta, -rho))
  *   O6 rank       (votes desc, index asc), keep K                                             (A11)
  *   O7 assign     PAPER.md L106 "hits that align with the straight line" -> nearest kept candidate
  *                 within the window, integer residual at the candidate's theta               (A12/A13)
