@@ -239,7 +239,8 @@ int hough_frontend_destroy(hough_frontend_t* fe);
 
 /* Enqueues the slicing on `stream` (no host synchronisation).
  *   d_x, d_y, d_z, d_t   [n_hits] fp32 RecoHits (mm, ns), structure of arrays
- *   d_fill_offsets       [n_fills + 1] int64, non-decreasing, fill f owns hits [fill_offsets[f], fill_offsets[f+1])
+ *   d_fill_offsets       [n_fills + 1] int64, non-decreasing, fill f owns hits [fill_offsets[f], fill_offsets[f+1]);
+ *                        a fill whose range does not lie inside [0, n_hits] is skipped and HOUGH_STATUS_BAD_OFFSETS is set
  *   d_u, d_v             [capacity] fp32 out: phi (degrees) and z of the windows' hits, window after window; inside a window
  *                        the hits keep their input order
  *   d_src                [capacity] int32 out: index of the input hit each output hit came from

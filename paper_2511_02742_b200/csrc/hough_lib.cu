@@ -986,7 +986,7 @@ int hough_frontend_slice(hough_frontend_t* fe, const float* d_x, const float* d_
         int blocks = (n_fills + 3) / 4;  // four warps per CTA, one warp per fill
         if (blocks > fe->n_sm * 16) blocks = fe->n_sm * 16;
         HOUGH_LAUNCH(hough::fe_scatter_kernel, blocks, 128, 0, st, fe->FP, d_z, reinterpret_cast<const long long*>(d_fill_offsets), n_fills,
-                     d_u, d_v, d_src, (long long)capacity);
+                     (long long)n_hits, d_u, d_v, d_src, (long long)capacity);
         HCK(cudaGetLastError());
     }
     return HOUGH_OK;

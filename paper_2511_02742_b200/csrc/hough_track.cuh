@@ -117,7 +117,7 @@ fe_scan_kernel(const FrontParams FP, long long n, long long* __restrict__ offset
 
 __global__ void __launch_bounds__(128)
 fe_scatter_kernel(const FrontParams FP, const float* __restrict__ z, const long long* __restrict__ fill_offsets, int n_fills,
-                  float* __restrict__ u_out, float* __restrict__ v_out, int* __restrict__ src_out, long long capacity)
+                  long long n_hits, float* __restrict__ u_out, float* __restrict__ v_out, int* __restrict__ src_out, long long capacity)
 {
     const int lane = threadIdx.x & 31;
     const int warp = (int)((blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5);
@@ -125,6 +125,8 @@ fe_scatter_kernel(const FrontParams FP, const float* __restrict__ z, const long 
     const unsigned lt = (1u << lane) - 1u;
     for (int f = warp; f < n_fills; f += n_warps) {
         const long long a = fill_offsets[f], b = fill_offsets[f + 1];
+        // fill offsets are caller data: a range outside [0, n_hits) would read window ranges that fe_count never wrote
+        if (a < 0 || b < a || b > n_hits) { if (lane == 0) atomicOr(FP.status, 2); continue; }
         volatile long long* cur = FP.cursor + (long long)f * FP.windows_per_fill;  // written by lane 0, read by all lanes of this warp
         for (long long i0 = a; i0 < b; i0 += 32) {
             const long long i = i0 + lane;

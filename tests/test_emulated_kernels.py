@@ -649,3 +649,16 @@ def test_an_event_that_ends_beyond_the_plans_hit_capacity_is_flagged_not_read(fl
     assert pe["status"] == 2 and pe["n_found"][2] == 0
     ts = E.two_stage(std_params(64, 64, T=8, K=4), b.u, b.v, offsets, 4, 4)
     assert ts["rc"] == 0 and ts["n_found"][2] == 0
+
+
+def test_frontend_skips_fills_whose_range_is_not_inside_the_hits():
+    """Fill offsets are caller data: a fill that starts below 0, ends before it starts or ends beyond n_hits is skipped and flagged
+    (BAD_OFFSETS); it is never used to index the per-hit scratch (found by tests/emu/fuzz_hostile.py: an endless loop otherwise)."""
+    fe = T.FrontEnd(windows_per_fill=6)
+    x, y, z, t, fo = synthetic_fills(4, seed=44)
+    n = len(x)
+    for bad in ([0, int(fo[1]), n + 100, int(fo[3]), n], [0, -5, int(fo[2]), int(fo[3]), n], [0, int(fo[2]), int(fo[1]), int(fo[3]), 2 ** 40]):
+        g = E.frontend_slice(fe, x, y, z, t, np.array(bad, np.int64))
+        assert g["status"] & 2
+    g = E.frontend_slice(fe, x, y, z, t, fo)                                 # and the honest offsets are not flagged
+    assert g["status"] == 0

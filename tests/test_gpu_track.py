@@ -110,6 +110,16 @@ def check_refit(cfg, n_events, geom):
         assert (fits[e, nk:]["n_hits"] == 0).all()
 
 
+def test_frontend_skips_fills_whose_range_is_not_inside_the_hits():
+    """Fill offsets are caller data: a fill that ends beyond n_hits, starts below 0 or ends before it starts is skipped and flagged."""
+    fe = T.FrontEnd(windows_per_fill=6)
+    x, y, z, t, fo = synthetic_fills(4, seed=44)
+    n = len(x)
+    for bad in ([0, int(fo[1]), n + 100, int(fo[3]), n], [0, -5, int(fo[2]), int(fo[3]), n], [0, int(fo[2]), int(fo[1]), int(fo[3]), 2 ** 40]):
+        assert gpu_slice(fe, x, y, z, t, np.array(bad, np.int64))[4] & H.HOUGH_STATUS_BAD_OFFSETS
+    assert gpu_slice(fe, x, y, z, t, fo)[4] == 0
+
+
 def test_refit_ignores_labels_beyond_the_kept_records():
     """Labels are caller data: one that names no kept record of its event must not index the per-candidate sums."""
     from test_emulated_kernels import fits_equal, GEOM
