@@ -101,6 +101,10 @@ def main():
         calls.append(("peeloff", L.hough_find_tracks_peeloff(h, du.ptr, dv.ptr, do.ptr, n_events, cands.ptr, nf.ptr, labels.ptr, None)))
         calls.append(("two_stage", L.hough_find_two_stage(h, du.ptr, dv.ptr, do.ptr, n_events, int(rng.choice([1, 2, 4])), int(rng.choice([1, 4, 8])),
                                                           cands.ptr, nf.ptr, None)))
+        # the host-buffer pipeline with the same garbage offsets (its own checks come first: offsets[0] must be 0, the total inside the plan)
+        hc, hn, hl = np.zeros((n_events, K), E.CAND_DTYPE), np.zeros(n_events, np.int32), np.zeros(max(n_hits, 1), np.int32)
+        calls.append(("run_host", L.hough_run_host_chunked(h, u.ctypes.data, v.ctypes.data, off.ctypes.data, n_events, hc.ctypes.data,
+                                                           hn.ctypes.data, hl.ctypes.data, int(rng.choice([0, 1, 3])))))
         dbg = np.zeros(16, np.uint64)
         L.hough_plan_debug_counters(h, dbg.ctypes.data, None)
         L.hough_plan_destroy(h)
