@@ -3,6 +3,7 @@ a long-running companion of tests/test_emulated_kernels.py, not part of the pyte
 
     python tests/emu/race_check.py [-k PYTEST_EXPRESSION] [--all] [--keep-logs DIR]
     python tests/emu/race_check.py --self-test       # the detector must FIND the race that a removed barrier opens
+    python tests/emu/race_check.py --fuzz N --seed S # N random plans of tests/emu/fuzz_parity.py instead of the pytest cases
 
 Builds tests/emu/libhough_emu_tsan.so (build_emu.py --tsan: the kernel sources compiled with -fsanitize=thread, every CUDA thread
 a detector fiber, the only happens-before edges inside a CTA being __syncthreads, __syncwarp and program order; atomics relaxed)
@@ -61,6 +62,8 @@ def main() -> int:
     ap.add_argument("--all", action="store_true", help="every case of tests/test_emulated_kernels.py")
     ap.add_argument("--keep-logs", default=None)
     ap.add_argument("--self-test", action="store_true")
+    ap.add_argument("--fuzz", type=int, default=0, help="run this many cases of fuzz_parity.py under the detector instead")
+    ap.add_argument("--seed", type=int, default=1)
     args = ap.parse_args()
     sys.path.insert(0, HERE)
     import build_emu
@@ -80,7 +83,9 @@ def main() -> int:
     env = dict(os.environ, LD_PRELOAD=libtsan, HOUGH_EMU_LIB=which, TSAN_OPTIONS=":".join(opts), OMP_NUM_THREADS="1",
                OPENBLAS_NUM_THREADS="1")
     cmd = [sys.executable, "-m", "pytest", os.path.join(ROOT, "tests", "test_emulated_kernels.py"), "-q", "-p", "no:cacheprovider"]
-    if not args.all:
+    if args.fuzz:
+        cmd = [sys.executable, os.path.join(HERE, "fuzz_parity.py"), "--cases", str(args.fuzz), "--seed", str(args.seed)]
+    elif not args.all:
         cmd += ["-k", args.k]
     rc = subprocess.call(cmd, env=env, cwd=ROOT)
     reports, first = 0, []
@@ -91,7 +96,7 @@ def main() -> int:
                 reports += 1
                 if len(first) < 3:
                     first.append("\n".join(block.splitlines()[:14]))
-    print(f"race_check: pytest exit code {rc}; ThreadSanitizer reports: {reports}; logs: {logdir}")
+    print(f"race_check: exit code of the cases {rc}; ThreadSanitizer reports: {reports}; logs: {logdir}")
     for b in first:
         print("----\n" + b)
     if args.self_test:
