@@ -211,7 +211,10 @@ hough_refit_kernel(const DevParams P, const PlaneParams G, const float* __restri
         for (long long i = g0 + tid; i < g1; i += nthr) {
             const int lab = labels[i];
             if (lab < 0 || lab >= nk) continue;  // unassigned or invalid hit; labels are caller data: one beyond the kept records is ignored
-            const int uq = __float2int_rn(__ldg(u + i) * P.hit_scale), vq = __float2int_rn(__ldg(v + i) * P.hit_scale);
+            const float uf = __ldg(u + i), vf = __ldg(v + i);
+            // assign never labels an invalid hit; a caller's label on one is ignored (its coordinates would break the exactness bound)
+            if (!(fabsf(uf) <= P.coord_max) || !(fabsf(vf) <= P.coord_max)) continue;
+            const int uq = __float2int_rn(uf * P.hit_scale), vq = __float2int_rn(vf * P.hit_scale);
             FitAcc& A = acc[lab];
             atomicAdd(&A.n, 1u);
             atomicAdd(&A.su, (unsigned long long)(long long)uq);

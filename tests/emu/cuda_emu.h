@@ -145,7 +145,13 @@ static inline void* emu_shared_ptr(unsigned addr, unsigned bytes, const char* wh
     }
     return cuda_emu::g_smem + off;
 }
-static inline int __float2int_rn(float x) { return (int)nearbyintf(x); }  // default rounding mode: ties to even
+static inline int __float2int_rn(float x)  // cvt.rni.s32.f32: ties to even, NaN -> 0, out of range saturates
+{
+    if (x != x) return 0;
+    if (x >= 2147483648.0f) return 2147483647;
+    if (x <= -2147483648.0f) return -2147483647 - 1;
+    return (int)nearbyintf(x);
+}
 static inline int __float_as_int(float x) { int i; memcpy(&i, &x, 4); return i; }
 static inline double __dmul_rn(double a, double b) { return a * b; }  // compiled with -ffp-contract=off
 static inline double __ddiv_rn(double a, double b) { return a / b; }
