@@ -13,7 +13,8 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 SOURCES = [os.path.join(_HERE, "csrc", "hough_lib.cu")]
-DEPENDS = SOURCES + [os.path.join(_HERE, "csrc", "hough_kernels.cuh"), os.path.join(_HERE, "csrc", "hough_fast.cuh"), os.path.join(_ROOT, "include", "hough.h")]
+# every file of csrc/ (hough_lib.cu includes all the .cuh headers) and the public header
+DEPENDS = sorted(os.path.join(_HERE, "csrc", f) for f in os.listdir(os.path.join(_HERE, "csrc"))) + [os.path.join(_ROOT, "include", "hough.h")]
 LIB = os.path.join(_HERE, "libhough.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -89,3 +89,19 @@ def test_product_never_imports_the_oracle():
     code = "import sys; import paper_2511_02742_b200.hough, paper_2511_02742_b200.synth; " \
            "assert not any(m == 'oracle' or m.startswith('oracle.') for m in sys.modules)"
     subprocess.check_call([sys.executable, "-c", code], cwd=ROOT)
+
+
+def test_the_build_step_depends_on_every_source_file():
+    """A header missing from build.DEPENDS means an edit to it does not rebuild libhough.so (round 2: hough_track.cuh was missing)."""
+    import os
+    from paper_2511_02742_b200 import build as b
+    csrc = os.path.join(os.path.dirname(b.__file__), "csrc")
+    deps = {os.path.abspath(d) for d in b.DEPENDS}
+    for f in os.listdir(csrc):
+        assert os.path.abspath(os.path.join(csrc, f)) in deps, f
+    assert any(d.endswith(os.path.join("include", "hough.h")) for d in deps)
+    # and every #include "..." of the translation unit is one of them
+    import re
+    for src in b.SOURCES:
+        for inc in re.findall(r'#include\s+"([^"]+)"', open(src).read()):
+            assert os.path.abspath(os.path.join(os.path.dirname(src), inc)) in deps, inc
