@@ -2,7 +2,7 @@
 the host CUDA model of cuda_emu.h.  TEST INFRASTRUCTURE -- NOT PART OF THE PRODUCT (nothing under paper_2511_02742_b200/
 imports or loads it).
 
-    python tests/emu/build_emu.py [--force] [--tsan | --ubsan]
+    python tests/emu/build_emu.py [--force] [--tsan | --ubsan | --no-bounds]
 
 --tsan builds tests/emu/libhough_emu_tsan.so, the race-detector variant: the kernel sources are compiled with
 -fsanitize=thread and -DHOUGH_EMU_TSAN (every CUDA thread a ThreadSanitizer fiber, see cuda_emu.cpp); the model itself
@@ -45,6 +45,21 @@ def build_tsan(force: bool = False, csrc: str = _CSRC, out: str = LIB_TSAN) -> s
 
 
 LIB_UBSAN = os.path.join(_HERE, "libhough_emu_ubsan.so")
+LIB_NOBOUNDS = os.path.join(_HERE, "libhough_emu_nobounds.so")
+
+
+def build_nobounds(force: bool = False) -> str:
+    """The host model WITHOUT -DHOUGH_BOUNDS: the kernels exactly as the product compiles them (the HB() checks are gone), with
+    only the model's guard pages and shared-window checks left.  An access that only HB() kept in range would fault here.
+    Use with HOUGH_EMU_LIB=tests/emu/libhough_emu_nobounds.so."""
+    if not force and os.path.exists(LIB_NOBOUNDS) and all(os.path.getmtime(d) <= os.path.getmtime(LIB_NOBOUNDS) for d in DEPENDS):
+        return LIB_NOBOUNDS
+    tmp = LIB_NOBOUNDS + f".tmp{os.getpid()}"
+    subprocess.check_call(["g++", "-std=c++17", "-O2", "-g", "-fPIC", "-shared", "-ffp-contract=off", "-fno-strict-aliasing", "-DHOUGH_EMU",
+                           "-Wno-unknown-pragmas", "-I", _HERE, "-x", "c++", os.path.join(_CSRC, "hough_lib.cu"),
+                           os.path.join(_HERE, "cuda_emu.cpp"), "-o", tmp, "-pthread"])
+    os.replace(tmp, LIB_NOBOUNDS)
+    return LIB_NOBOUNDS
 
 
 def build_ubsan(force: bool = False) -> str:
@@ -75,4 +90,5 @@ def build(force: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print((build_tsan if "--tsan" in sys.argv else build_ubsan if "--ubsan" in sys.argv else build)(force="--force" in sys.argv))
+    which = build_tsan if "--tsan" in sys.argv else build_ubsan if "--ubsan" in sys.argv else build_nobounds if "--no-bounds" in sys.argv else build
+    print(which(force="--force" in sys.argv))
