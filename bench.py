@@ -218,6 +218,11 @@ def run_ours(args, cfg=None, hits_idx=None, grid_idx=None, quiet=False):
 
     import torch
     from paper_2511_02742_b200 import hough as H
+    from paper_2511_02742_b200 import build as hough_build
+    try:
+        hough_build.build()                                        # no-op unless libhough.so is missing or older than its sources
+    except Exception as exc:  # noqa: BLE001  (no nvcc: the load below then says what is missing)
+        print(f"bench.py: libhough.so was not (re)built: {exc}", file=sys.stderr)    # (every rank: the output is replaced atomically)
     H.load_library()                                               # raises if libhough.so is not built: no fallback
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)

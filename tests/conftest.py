@@ -23,6 +23,14 @@ def pytest_configure(config):
     if variant:
         from paper_2511_02742_b200 import build, hough
         hough.load_library(build.build(variant=variant))
+    else:
+        # a fresh checkout has no libhough.so (built artefacts are not in the history): build it now if it is missing or older than
+        # its sources -- a no-op otherwise.  Without nvcc nothing is built, and the binding still fails loudly when a test loads it.
+        try:
+            from paper_2511_02742_b200 import build
+            build.build()
+        except Exception as exc:  # noqa: BLE001
+            print(f"conftest: libhough.so was not (re)built: {exc}", file=sys.stderr)
 
 
 def pytest_collection_modifyitems(config, items):
