@@ -53,7 +53,7 @@ typedef enum {
 enum { HOUGH_I32 = 0, HOUGH_U16 = 1 };            /* count_dtype: element type of accumulators dumped by hough_vote */
 enum { HOUGH_STATUS_EVENT_TOO_LONG = 1, HOUGH_STATUS_BAD_OFFSETS = 2,      /* bits of the device status word */
        HOUGH_STATUS_INTERNAL = 4 };   /* set only by the -DHOUGH_BOUNDS debug build: an index check inside a kernel failed */
-/* hough_plan_desc_t.flags.  Both change only WHICH kernel computes an event, never a result:
+/* hough_plan_desc_t.flags.  The first two change only WHICH kernel computes an event, never a result:
  *   HOUGH_FLAG_GENERAL_ONLY  every event goes through the general kernel (the shared-memory-only fast kernel is not used)
  *   HOUGH_FLAG_SMALL_LISTS   the fast kernel's per-event lists get their smallest capacities, so that ordinary events
  *                            overflow them and are handed to the general kernel (exercises that hand-over in tests) */
