@@ -105,3 +105,26 @@ def test_the_build_step_depends_on_every_source_file():
     for src in b.SOURCES:
         for inc in re.findall(r'#include\s+"([^"]+)"', open(src).read()):
             assert os.path.abspath(os.path.join(os.path.dirname(src), inc)) in deps, inc
+
+
+def test_enumerators_of_the_header_match_the_binding():
+    """Every HOUGH_* enumerator with an explicit value in include/hough.h has the same value in the Python binding (and in the
+    host-model driver of the tests)."""
+    import os
+    import re
+    import sys
+    from paper_2511_02742_b200 import hough as H
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    text = re.sub(r"/\*.*?\*/", " ", open(os.path.join(root, "include", "hough.h")).read(), flags=re.S)
+    found = {name: int(val) for name, val in re.findall(r"\b(HOUGH_[A-Z0-9_]+)\s*=\s*(-?\d+)", text)}
+    assert {"HOUGH_FLAG_THETA_WRAP", "HOUGH_STATUS_BAD_OFFSETS", "HOUGH_U16", "HOUGH_FIT_FOUND", "HOUGH_EINVAL"} <= set(found)
+    checked = 0
+    for name, val in found.items():
+        if hasattr(H, name):
+            assert getattr(H, name) == val, name
+            checked += 1
+    assert checked >= 10
+    sys.path.insert(0, os.path.join(root, "tests", "emu"))
+    import hough_emu as E
+    assert (E.FLAG_GENERAL_ONLY, E.FLAG_SMALL_LISTS, E.FLAG_THETA_WRAP) == (found["HOUGH_FLAG_GENERAL_ONLY"], found["HOUGH_FLAG_SMALL_LISTS"], found["HOUGH_FLAG_THETA_WRAP"])
+    assert (E.HOUGH_I32, E.HOUGH_U16) == (found["HOUGH_I32"], found["HOUGH_U16"])
